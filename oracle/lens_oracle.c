@@ -1,0 +1,221 @@
+/*
+ * lens_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, single-threaded, double-precision CPU statement of what the
+ * lens-map hot path computes.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may call it.  It shares no
+ * code, header, table or constant with the CUDA path under
+ * paper_2004_06352_b200/csrc (it even declares its own lens record).
+ *
+ * Build: gcc -O2 -ffp-contract=off -fPIC -shared lens_oracle.c -lm
+ *        (no FMA contraction, so results do not depend on the host ISA).
+ *
+ * What it follows (PAPER.md = /root/reference/PAPER.md, arXiv 2004.06352):
+ *   - alpha = grad psi, lens equation            PAPER.md:39-53  (eq. 1-2)
+ *   - A^-1 = delta_ij - d_ij psi, kappa, gamma   PAPER.md:57     (eq. 4)
+ *   - mu = 1/det A^-1                            PAPER.md:64     (eq. 5)
+ *   - kappa/gamma/mu maps from 2nd derivatives   PAPER.md:105-110 (eq. 7-9)
+ *   - "at each grid-point the second-order derivative contribution of each
+ *      cluster member is added up"               PAPER.md:112    (sec. 2.4)
+ *   - grad phi = sum_h grad phi_h                PAPER.md:183    (eq. 10)
+ * The paper never prints the potentials (PAPER.md:70 only names the parameter
+ * kinds and cites ref [6]); the per-lens closed forms are the
+ * reading fixed in SURVEY.md sec. 8(c) / Appendix A.1-A.3 and DESIGN.md sec. 3:
+ * a PIEMD of core r has convergence kappa = 1/(2 sqrt(r^2 + rho^2)),
+ * rho^2 = x'^2/(1+eps)^2 + y'^2/(1-eps)^2; NSIE = b0*PIEMD(rcore);
+ * dPIE = b0*rcut/(rcut-rcore)*(PIEMD(rcore) - PIEMD(rcut)); SIS = circular,
+ * r = 0.  Garbled equations are read as DESIGN.md sec. 3 lists (eq. 8: sum the
+ * Hessian first, gamma1 = (a11-a22)/2, gamma2 = a12; eq. 9: minus sign).
+ *
+ * The dPIE is written in its straightforward two-term form (core term minus
+ * cut term, libm atan/atanh/sqrt, explicit rotation matrices) -- deliberately
+ * NOT the merged / rotation-free forms the GPU uses.
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"): Poisson integral of kappa
+ * by quadrature, SURVEY Appendix B 40-digit worked example, circular dPIE and
+ * SIS closed forms, linearity, finite-difference Hessian, epilogue identities,
+ * rotation covariance, limits between types, far-field mass, mpmath
+ * complex-log brute force.  No function here is "parity unpinned".
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+
+enum { ORC_DPIE = 0, ORC_NSIE = 1, ORC_SIS = 2 };
+
+/* own declaration of the 64-byte boundary record (same bytes as lh_lens) */
+typedef struct {
+    int32_t type;
+    int32_t pad_;
+    double x, y;        /* centre [arcsec] */
+    double ellipticity; /* e-hat = (A^2-B^2)/(A^2+B^2) of the isodensities */
+    double theta;       /* major axis, CCW from +x [rad] */
+    double rcore, rcut; /* [arcsec] */
+    double b0;          /* [arcsec] */
+} orc_lens;
+
+/* first and second derivatives of one potential: (ax, ay, a11, a12, a22) */
+typedef struct {
+    double ax, ay, a11, a12, a22;
+} orc_deriv;
+
+/* Reading 8c-2: eps = e-hat / (1 + sqrt(1 - e-hat^2)) */
+double orc_eps_from_ehat(double ehat) { return ehat / (1.0 + sqrt(1.0 - ehat * ehat)); }
+
+/*
+ * PIEMD kernel with core r and unit b0 in the LENS frame (Appendix A.1):
+ *   Jx = o/(2 sqrt(eps)) * atan ( 2 sqrt(eps) x' / (o w + (1+eps)^2 r) )
+ *   Jy = o/(2 sqrt(eps)) * atanh( 2 sqrt(eps) y' / (o w + (1-eps)^2 r) )
+ *   D  = 2(1+eps^2) r^2 + 2 o r w + x'^2 + y'^2
+ *   hxx = ((1-eps)^2 r^2 + o r w + y'^2)/(w D)
+ *   hyy = ((1+eps)^2 r^2 + o r w + x'^2)/(w D)
+ *   hxy = -x' y'/(w D)
+ * with o = 1 - eps^2, w = sqrt(r^2 + rho^2).  eps -> 0 (A.2): atan(u)/u -> 1.
+ */
+static void piemd_kernel(double xp, double yp, double eps, double r, double *jx, double *jy, double *hxx,
+                         double *hxy, double *hyy) {
+    const double o = 1.0 - eps * eps;
+    const double p = (1.0 + eps) * (1.0 + eps);
+    const double m = (1.0 - eps) * (1.0 - eps);
+    const double rho2 = xp * xp / p + yp * yp / m;
+    const double w = sqrt(r * r + rho2);
+    const double se2 = 2.0 * sqrt(eps);
+
+    const double X = xp / (o * w + p * r); /* atan argument / (2 sqrt eps) */
+    const double Y = yp / (o * w + m * r); /* atanh argument / (2 sqrt eps) */
+    const double ux = se2 * X, uy = se2 * Y;
+    /* o/(2 sqrt eps) * atan(ux) == o * X * (atan(ux)/ux); the ratio is 1 at ux = 0 */
+    const double atanc = (ux != 0.0) ? atan(ux) / ux : 1.0;
+    const double atanhc = (uy != 0.0) ? atanh(uy) / uy : 1.0;
+    *jx = o * X * atanc;
+    *jy = o * Y * atanhc;
+
+    const double D = 2.0 * (1.0 + eps * eps) * r * r + 2.0 * o * r * w + xp * xp + yp * yp;
+    const double wD = w * D;
+    *hxx = (m * r * r + o * r * w + yp * yp) / wD;
+    *hyy = (p * r * r + o * r * w + xp * xp) / wD;
+    *hxy = -xp * yp / wD;
+}
+
+/* One potential at one point.  Types and rotation: Appendix A.3, readings 8c-1,3,11,19. */
+void orc_lens_deriv(const orc_lens *L, double X, double Y, orc_deriv *out) {
+    const double dx = X - L->x, dy = Y - L->y;
+    out->ax = out->ay = out->a11 = out->a12 = out->a22 = 0.0;
+
+    if (L->type == ORC_SIS) {
+        /* alpha = b0 (dx,dy)/R ; H = b0/R^3 [[dy^2, -dx dy],[-dx dy, dx^2]] ; zero at R = 0 */
+        const double R2 = dx * dx + dy * dy;
+        if (R2 == 0.0) return;
+        const double R = sqrt(R2);
+        out->ax = L->b0 * dx / R;
+        out->ay = L->b0 * dy / R;
+        const double R3 = R2 * R;
+        out->a11 = L->b0 * dy * dy / R3;
+        out->a12 = -L->b0 * dx * dy / R3;
+        out->a22 = L->b0 * dx * dx / R3;
+        return;
+    }
+
+    const double c = cos(L->theta), s = sin(L->theta);
+    const double xp = c * dx + s * dy;  /* lens frame: x' along the major axis */
+    const double yp = -s * dx + c * dy;
+    const double eps = orc_eps_from_ehat(L->ellipticity);
+
+    double jx, jy, hxx, hxy, hyy; /* lens-frame alpha' and H' */
+    if (L->type == ORC_NSIE) {
+        piemd_kernel(xp, yp, eps, L->rcore, &jx, &jy, &hxx, &hxy, &hyy);
+        jx *= L->b0; jy *= L->b0; hxx *= L->b0; hxy *= L->b0; hyy *= L->b0;
+    } else { /* ORC_DPIE: core term minus cut term */
+        double jxc, jyc, hxxc, hxyc, hyyc, jxt, jyt, hxxt, hxyt, hyyt;
+        piemd_kernel(xp, yp, eps, L->rcore, &jxc, &jyc, &hxxc, &hxyc, &hyyc);
+        piemd_kernel(xp, yp, eps, L->rcut, &jxt, &jyt, &hxxt, &hxyt, &hyyt);
+        const double T = L->b0 * L->rcut / (L->rcut - L->rcore);
+        jx = T * (jxc - jxt);
+        jy = T * (jyc - jyt);
+        hxx = T * (hxxc - hxxt);
+        hxy = T * (hxyc - hxyt);
+        hyy = T * (hyyc - hyyt);
+    }
+    /* back-rotation alpha = R(theta) alpha', H = R H' R^T */
+    out->ax = c * jx - s * jy;
+    out->ay = s * jx + c * jy;
+    out->a11 = c * c * hxx - 2.0 * c * s * hxy + s * s * hyy;
+    out->a22 = s * s * hxx + 2.0 * c * s * hxy + c * c * hyy;
+    out->a12 = c * s * (hxx - hyy) + (c * c - s * s) * hxy;
+}
+
+/* Superposition in lens-index order (eq. 10; sec. 2.4). */
+void orc_point(const orc_lens *lenses, int nlens, double X, double Y, orc_deriv *sum) {
+    orc_deriv acc = {0.0, 0.0, 0.0, 0.0, 0.0};
+    for (int l = 0; l < nlens; ++l) {
+        orc_deriv d;
+        orc_lens_deriv(&lenses[l], X, Y, &d);
+        acc.ax += d.ax;
+        acc.ay += d.ay;
+        acc.a11 += d.a11;
+        acc.a12 += d.a12;
+        acc.a22 += d.a22;
+    }
+    *sum = acc;
+}
+
+/* Epilogue (eq. 4, 5, 7-9 as read in DESIGN.md sec. 3; Appendix A.6). */
+void orc_epilogue(double a11, double a12, double a22, double *kappa, double *gamma1, double *gamma2, double *mu) {
+    const double k = 0.5 * (a11 + a22);
+    const double g1 = 0.5 * (a11 - a22);
+    const double g2 = a12;
+    const double det = (1.0 - k) * (1.0 - k) - g1 * g1 - g2 * g2;
+    *kappa = k;
+    *gamma1 = g1;
+    *gamma2 = g2;
+    *mu = 1.0 / det; /* IEEE: +-inf on a critical line */
+}
+
+/* the nine output planes; a NULL plane is not written */
+typedef struct {
+    double *ax, *ay, *a11, *a12, *a22, *kappa, *gamma1, *gamma2, *mu;
+} orc_planes;
+
+static void store(const orc_planes *o, size_t idx, const orc_deriv *d) {
+    double k, g1, g2, mu;
+    orc_epilogue(d->a11, d->a12, d->a22, &k, &g1, &g2, &mu);
+    if (o->ax) o->ax[idx] = d->ax;
+    if (o->ay) o->ay[idx] = d->ay;
+    if (o->a11) o->a11[idx] = d->a11;
+    if (o->a12) o->a12[idx] = d->a12;
+    if (o->a22) o->a22[idx] = d->a22;
+    if (o->kappa) o->kappa[idx] = k;
+    if (o->gamma1) o->gamma1[idx] = g1;
+    if (o->gamma2) o->gamma2[idx] = g2;
+    if (o->mu) o->mu[idx] = mu;
+}
+
+/* arbitrary points: out planes hold npts values each */
+void orc_points(const orc_lens *lenses, int nlens, const double *xs, const double *ys, size_t npts,
+                const orc_planes *o) {
+    for (size_t k = 0; k < npts; ++k) {
+        orc_deriv d;
+        orc_point(lenses, nlens, xs[k], ys[k], &d);
+        store(o, k, &d);
+    }
+}
+
+/*
+ * Rows [j0, j1) of the regular grid: pixel (i, j) at (x0 + i*dx, y0 + j*dx),
+ * plane index j*nx + i ("rectangular grid ... each grid cell the
+ * size of a pixel"; reading 8c-10).  Planes are FULL ny*nx maps; only the row
+ * range is written, so disjoint ranges can run on different host threads.
+ */
+void orc_grid_rows(const orc_lens *lenses, int nlens, double x0, double y0, double dx, int nx, int ny, int j0,
+                   int j1, const orc_planes *o) {
+    (void)ny;
+    for (int j = j0; j < j1; ++j) {
+        const double Y = y0 + (double)j * dx;
+        for (int i = 0; i < nx; ++i) {
+            const double X = x0 + (double)i * dx;
+            orc_deriv d;
+            orc_point(lenses, nlens, X, Y, &d);
+            store(o, (size_t)j * (size_t)nx + (size_t)i, &d);
+        }
+    }
+}
