@@ -1,0 +1,302 @@
+#!/usr/bin/env python
+"""bench.py -- pixel-lens FP64 gradient+Hessian evaluations per second on B200.
+
+A "step" is one pass of the whole hot path (rows a1-a5: pack the lens
+list, stage the table, superpose first and second derivatives over all lenses at every
+pixel, fused kappa/gamma/mu epilogue, stores) over BASELINE.json config 3:
+4096 x 4096 pixels x 1000 dPIE potentials, outputs ax ay kappa gamma1 gamma2 mu, the
+Hessian never written.  One process per GPU; at N > 1 every rank evaluates its own lens
+model (an MCMC-style independent sample) on the same grid -- the path shards by
+independent problems with no exchange step, so there is no collective on the data path
+and `scaling` is "weak".
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/) on the
+host cores on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import lens_inputs as li  # noqa: E402
+
+METRIC = "pixel-lens FP64 gradient+Hessian evals/sec"
+UNIT = "evals/s"
+
+# Executed FP64 flops per (pixel, lens) evaluation of the timed kernel variant (gradient +
+# Hessian, dPIE), from the ncu counters (2*dfma + dadd + dmul thread-instructions) / evals:
+# profiles/r01_ncu_cfg3.md.  DESIGN.md sec. 7 derives the same figure from the SASS.
+FLOPS_PER_EVAL = {"grad+hess": 0.0, "grad": 0.0, "hess": 0.0}
+# SURVEY.md sec. 8(d) canonical count for the cheapest exact formulation it knew (context)
+CANONICAL_FLOPS_PER_EVAL = {"grad+hess": 278.0, "grad": 205.0, "hess": 105.0}
+# FP64 CUDA-core peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x SM clock (B200_PROFILING.md:
+# 148 SMs, clocks.max.sm 1965 MHz).  The live DFMA probe (lh_fp64_peak_probe) is the
+# measured counterpart and is what `roofline.peak` reports.
+NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# dram bytes (read+write) per launch of the timed kernel from `ncu --set full` (profiles/); None until captured
+NCU_TRAFFIC_BYTES = {3: None}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (bench line: 3)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------- CPU oracle leg
+def oracle_sample(cfg, seconds: float):
+    """Time the oracle as it stands on a bounded sample: whole rows of the configured grid,
+    all lenses, all host cores (threads over disjoint row ranges)."""
+    import oracle
+
+    cores = os.cpu_count() or 1
+    g, L = cfg.grid, cfg.lenses[: cfg.nlens]
+    t0 = time.perf_counter()
+    oracle.grid(L, g.x0, g.y0, g.dx, g.nx, g.ny, planes=cfg.outputs, threads=cores, rows=(0, cores))
+    rate = cores * g.nx * cfg.nlens / (time.perf_counter() - t0)  # evals/s, all cores, rough
+    rows = int(max(cores, min(g.ny, seconds * rate / (g.nx * cfg.nlens))))
+    rows = max(cores, rows // cores * cores)
+    t0 = time.perf_counter()
+    oracle.grid(L, g.x0, g.y0, g.dx, g.nx, g.ny, planes=cfg.outputs, threads=cores, rows=(0, rows))
+    dt = time.perf_counter() - t0
+    evals = rows * g.nx * cfg.nlens
+    return {"value": evals / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"rows 0..{rows - 1} of the {g.nx}x{g.ny} grid x {cfg.nlens} lenses "
+                      f"({evals:.3g} evals, {dt:.1f} s; oracle/lens_oracle.c single-threaded per row slab, "
+                      f"{cores} slabs in parallel)"}, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = li.config(args.config)
+    per_step = max(1.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(cfg, per_step / 4)
+    vals, times = [], []
+    base = None
+    for _ in range(args.steps):
+        base, dt = oracle_sample(cfg, per_step)
+        vals.append(base["value"]); times.append(dt)
+    v = float(np.mean(vals))
+    base["value"] = v
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(cfg, args), "cpu_baseline": base,
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, args):
+    g = cfg.grid
+    return {"workload": f"BASELINE.json configs[{args.config}] {cfg.name}: {g.nx}x{g.ny} px, {cfg.nlens} lenses"
+                        + (f" x {cfg.nmodel} models" if cfg.nmodel > 1 else ""),
+            "outputs": list(cfg.outputs), "evals_per_step_per_gpu": cfg.evals,
+            "l2": "output planes (%d MiB/step) exceed the 126 MB L2 and a 256 MiB buffer is rewritten between "
+                  "timed steps; the lens table (%d KiB) is cache-resident by design"
+                  % (len(cfg.outputs) * cfg.nmodel * g.npix * 8 >> 20, cfg.nmodel * cfg.nlens * 224 >> 10),
+            "parallelism": f"independent lens models per GPU x{args.gpus}, no collective"}
+
+
+# ----------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2004_06352_b200 as lh
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = li.config(args.config)
+    g = cfg.grid
+    lenses = cfg.lenses
+    if world > 1 and rank > 0 and cfg.nmodel == 1:
+        # another independent sample of the same model family for this rank (same shape, other seed)
+        lenses = li.cluster(1000 * args.config + rank, {1: 2, 2: 3, 3: 4}.get(args.config, 0), cfg.nlens
+                            - {1: 2, 2: 3, 3: 4}.get(args.config, 0), {0: 40.0, 3: 150.0}.get(args.config, 100.0))
+    shape = (cfg.nmodel, g.ny, g.nx)
+    out = {n: torch.empty(shape, dtype=torch.float64, device="cuda") for n in cfg.outputs}
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+    lh.lh_set_stream(stream)
+
+    def step():
+        lh.lh_grid_eval_batch(lenses, cfg.nmodel, cfg.nlens, g, **out)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    launches0 = lh.lh_launch_count()
+    with ClockSampler(local) as clk:
+        barrier()
+        for a, b in ev:
+            flush.zero_()  # L2 flush, outside the timed events
+            a.record(stream)
+            step()
+            b.record(stream)
+        barrier()
+    launches = lh.lh_launch_count() - launches0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * cfg.evals / (ms_per_step * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        host = {n: torch.empty(shape, dtype=torch.float64).pin_memory() for n in cfg.outputs}
+        def step_host():
+            lh.lh_grid_eval_host(lenses, cfg.nmodel, cfg.nlens, g, **host)
+        step_host()
+        barrier()
+        t0 = time.perf_counter()
+        k_e2e = max(1, min(args.steps, 3))
+        for _ in range(k_e2e):
+            step_host()  # synchronises its stream before returning
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * cfg.evals * k_e2e / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(cfg.nmodel * cfg.nlens * 224 + cfg.nmodel * 16),
+               "d2h_bytes_per_step": int(len(cfg.outputs) * cfg.nmodel * g.npix * 8),
+               "ms_per_step": 1e3 * dt / k_e2e, "steps": k_e2e,
+               "note": "lh_grid_eval_host: host lens list in, pinned host planes out, packing + copies + sync timed"}
+        del host
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant (only) kernel: FP64 CUDA-core ALU bound
+    peak_flops, _ = lh.lh_fp64_peak_probe(1 << 15)
+    mode = "grad+hess" if (set(cfg.outputs) & {"ax", "ay"}) and (set(cfg.outputs) - {"ax", "ay"}) else (
+        "grad" if set(cfg.outputs) <= {"ax", "ay"} else "hess")
+    fpe = FLOPS_PER_EVAL[mode] or CANONICAL_FLOPS_PER_EVAL[mode]
+    kernel_s = float(np.mean(step_ms)) * 1e-3
+    achieved = fpe * cfg.evals / kernel_s / 1e12
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak_flops / 1e12, "unit": "TFLOP/s",
+                "frac": achieved / (peak_flops / 1e12), "traffic": NCU_TRAFFIC_BYTES.get(args.config),
+                "peak_source": "measured live: lh_fp64_peak_probe (DFMA chains, all SMs); nominal "
+                               f"{NOMINAL_FP64_TFLOPS:.1f} TFLOP/s = 148 SM x 64 lanes x 2 x 1.965 GHz",
+                "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
+                "flops_per_eval": fpe, "flops_per_eval_source": "ncu-counted executed FP64 flops" if
+                FLOPS_PER_EVAL[mode] else "SURVEY 8(d) canonical count (no ncu count yet)",
+                "canonical_flops_per_eval": CANONICAL_FLOPS_PER_EVAL[mode],
+                "achieved_canonical": CANONICAL_FLOPS_PER_EVAL[mode] * cfg.evals / kernel_s / 1e12,
+                "kernel_ms": kernel_s * 1e3, "kernel": "lh::superpose_kernel<%s>" % mode,
+                "store_gbs": len(cfg.outputs) * cfg.nmodel * g.npix * 8 / kernel_s / 1e9}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args),
+            "clocks": clk.summary(), "gpu_launches": int(launches), "roofline": roofline}
+    if e2e:
+        line["e2e"] = e2e
+    if not args.no_cpu_baseline and world >= 1:
+        line["cpu_baseline"], _ = oracle_sample(cfg, args.cpu_seconds)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

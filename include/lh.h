@@ -1,0 +1,155 @@
+/*
+ * lh.h -- C ABI of liblh.so: the lens-map hot path of Lenstool-HPC
+ * (arXiv 2004.06352), built from scratch for NVIDIA B200 (sm_100a), FP64.
+ *
+ * What the library computes.  For every pixel of a regular image-plane grid
+ * ("a rectangular grid defined on the image-plane, each grid cell usually being
+ * the size of a pixel", PAPER.md:99 sec. 2.4; :181 sec. 4.1) and a list of N
+ * parametric potentials (sec. 2.2):
+ *
+ *   - the deflection alpha = grad psi as the sum of the first derivatives of all
+ *     potentials at that point (PAPER.md:183 eq. 10; :53 alpha = grad psi);
+ *   - the second derivatives a_ij = d_ij psi, "at each grid-point the
+ *     second-order derivative contribution of each cluster member is added up"
+ *     (sec. 2.4);
+ *   - the maps kappa = (a11+a22)/2, gamma1 = (a11-a22)/2, gamma2 = a12,
+ *     mu = 1/((1-kappa)^2 - gamma1^2 - gamma2^2)
+ *     (PAPER.md:57 eq. 4, :64 eq. 5, :105-110 eq. 7-9; garbled signs/sums read as
+ *     DESIGN.md sec. 3 states).
+ *
+ * The paper does not print the potentials; the profiles (dPIE = difference of two
+ * PIEMDs, NSIE, SIS), their normalisation and the ellipticity / angle conventions
+ * are the readings listed in DESIGN.md sec. 3.
+ *
+ * Conventions common to every call
+ *   units      arcsec for lengths, radians for theta; all reals IEEE binary64.
+ *   lenses     HOST pointer, caller-owned, read only during the call (packed and
+ *              copied before return; may be freed or changed right after).
+ *   grid       HOST pointer, read during the call.
+ *   outputs    DEVICE pointers (cudaMalloc / torch CUDA tensor .data_ptr()),
+ *              caller-owned, 8-byte aligned, ny*nx doubles each (times nmodel for
+ *              batch calls), row-major: pixel (i, j) at (x0 + i*dx, y0 + j*dx) is
+ *              element j*nx + i; model m starts at m*ny*nx.  Fully overwritten.
+ *              The *_host entry points take HOST pointers instead.
+ *   stream     work is enqueued on the stream set by lh_set_stream() for the
+ *              calling host thread (default: the legacy default stream) and the
+ *              call returns without synchronising the device.  (The *_host entry
+ *              points synchronise that stream before they return.)
+ *   errors     0 on success.  A negative code on failure, in which case no
+ *              output element has been written; lh_last_error() gives a message.
+ *              No exception or abort crosses this boundary.
+ *   nlens = 0  is valid: alpha = 0, a_ij = 0, kappa = gamma = 0, mu = 1.
+ *   IEEE       mu = +-inf where det A^-1 == 0 exactly.  A pixel that coincides
+ *              exactly with the centre of an SIS gets zero contribution from it.
+ */
+#ifndef LH_H_
+#define LH_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LH_OK 0
+#define LH_EINVAL (-1) /* bad argument; nothing was enqueued */
+#define LH_ECUDA (-2)  /* a CUDA call failed; see lh_last_error() */
+
+enum { LH_DPIE = 0, LH_NSIE = 1, LH_SIS = 2 };
+
+/* One parametric potential, 64 bytes (AoS at the boundary; the library packs to a
+ * per-lens table of precomputed constants, sorted by type, on the device). */
+typedef struct {
+    int32_t type;       /* LH_DPIE, LH_NSIE or LH_SIS */
+    int32_t _pad;       /* ignored */
+    double x, y;        /* centre */
+    double ellipticity; /* e-hat = (A^2-B^2)/(A^2+B^2) of the mass isodensities, in [0,1); ignored for SIS */
+    double theta;       /* position angle of the major axis, CCW from +x; ignored for SIS */
+    double rcore;       /* dPIE: 0 < rcore < rcut; NSIE: > 0; SIS: ignored */
+    double rcut;        /* dPIE only */
+    double b0;          /* = (D_ls/D_s) 6 pi (sigma/c)^2 in arcsec, finite (SIS: |alpha| = b0) */
+} lh_lens;
+
+/* Regular grid with square pixels: pixel (i, j) at (x0 + i*dx, y0 + j*dx). */
+typedef struct {
+    double x0, y0, dx;
+    int32_t nx, ny;
+} lh_grid;
+
+/* Up to nine output planes; NULL = not wanted (and then never touched). */
+typedef struct {
+    double *ax, *ay;                     /* deflection           (eq. 10) */
+    double *a11, *a12, *a22;             /* Hessian of psi       (sec. 2.4) */
+    double *kappa, *gamma1, *gamma2, *mu; /* maps                 (eq. 4, 5, 7-9) */
+} lh_outputs;
+
+/* alpha_x, alpha_y on the grid (eq. 10).  Both planes required.
+ * LH_EINVAL: NULL pointer, nlens < 0, nx or ny <= 0, nx*ny >= 2^40, dx <= 0 or
+ * non-finite x0/y0/dx, unknown lens type, non-finite parameter, e-hat outside [0,1),
+ * dPIE with rcore <= 0 or rcut <= rcore, NSIE with rcore <= 0, output pointer that
+ * is not device memory or not 8-byte aligned. */
+int lh_grid_gradient(const lh_lens *lenses, int nlens, const lh_grid *g, double *out_ax, double *out_ay);
+
+/* a11 = d_xx psi, a12 = d_xy psi, a22 = d_yy psi summed over lenses.
+ * All three planes required.  Errors as above. */
+int lh_grid_hessian(const lh_lens *lenses, int nlens, const lh_grid *g, double *a11, double *a12, double *a22);
+
+/* kappa, gamma1, gamma2, mu (PAPER.md:57-64 eq. 4-5; :105-110 eq. 7-9).  All four
+ * planes required.  The Hessian is reduced in registers and never written. */
+int lh_lens_maps(const lh_lens *lenses, int nlens, const lh_grid *g, double *kappa, double *gamma1, double *gamma2,
+                 double *mu);
+
+/* Deflection maps of `nmodel` lens models on one shared grid in one launch -- the
+ * shape in which an MCMC sampler or the map-variance computation issues them
+ * (PAPER.md:81 sec. 2.2; :101, :114 sec. 2.4).  lenses[m*nlens + l] is lens l of
+ * model m; out_ax[m*ny*nx + j*nx + i].  nmodel >= 1, nmodel*nx*ny < 2^40. */
+int lh_grid_gradient_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *out_ax,
+                           double *out_ay);
+
+/* Any subset of the nine planes in ONE pass over the lenses (at least one plane
+ * must be non-NULL).  The four calls above are thin wrappers of this one. */
+int lh_grid_eval(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_outputs *o);
+
+/* Batched form of lh_grid_eval (layout as lh_grid_gradient_batch). */
+int lh_grid_eval_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *o);
+
+/* Same as lh_grid_eval_batch with HOST output planes: the library allocates (and
+ * caches) device planes, runs the same kernel, copies the requested planes back
+ * and synchronises the stream before returning.  This is the end-to-end path a
+ * caller without device buffers uses. */
+int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *host_o);
+
+/* CUDA stream (a cudaStream_t / CUstream cast to void*) used by later calls from
+ * this host thread; NULL = legacy default stream.  Always returns LH_OK. */
+int lh_set_stream(void *cuda_stream);
+
+/* Message for the last non-zero return on this host thread ("" if none). */
+const char *lh_last_error(void);
+
+/* Number of kernels this host thread has launched through the library so far. */
+long long lh_launch_count(void);
+
+/* Step a1 on its own (host only, no CUDA call): validate `n` lenses of one model and
+ * write the per-lens constant table the kernels consume -- n records of
+ * LH_PACK_DOUBLES doubles, sorted by evaluation class (stable inside a class) -- into
+ * host memory `table`, and the class boundaries into class_begin[0..LH_PACK_CLASSES]
+ * (class k = records [class_begin[k], class_begin[k+1])).  `table` may be NULL to
+ * validate only.  Returns LH_OK or LH_EINVAL (rules as lh_grid_gradient). */
+#define LH_PACK_DOUBLES 28
+#define LH_PACK_CLASSES 3
+int lh_pack_model(const lh_lens *lenses, int n, double *table, int32_t *class_begin);
+
+/* Diagnostic: runs a register-resident chain of dependent-free FP64 FMAs on every
+ * SM for `iters` iterations and returns the achieved FP64 FLOP/s in *flops_per_s
+ * (2 per FMA) and the kernel time in *seconds (CUDA events on the set stream;
+ * synchronises).  Used by bench.py as the measured FP64 CUDA-core roofline. */
+int lh_fp64_peak_probe(int iters, double *flops_per_s, double *seconds);
+
+/* "lh <major>.<minor> sm_100a" */
+const char *lh_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LH_H_ */

@@ -1,0 +1,224 @@
+"""paper_2004_06352_b200 -- thin Python binding of liblh.so (include/lh.h).
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels
+behind the C ABI.  PyTorch is used by callers for device memory and streams; this
+module needs nothing but ctypes + numpy and fails loudly when the CUDA library is
+missing -- there is no CPU fallback (and it never imports `oracle`).
+
+Names mirror the C ABI one to one:
+    lh_grid_gradient, lh_grid_hessian, lh_lens_maps, lh_grid_gradient_batch,
+    lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_pack_model, lh_set_stream,
+    lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_version
+Outputs may be torch CUDA tensors (float64, contiguous), anything with a
+`data_ptr()`, or raw integer device addresses.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import _build
+
+LH_OK, LH_EINVAL, LH_ECUDA = 0, -1, -2
+LH_DPIE, LH_NSIE, LH_SIS = 0, 1, 2
+PLANES = ("ax", "ay", "a11", "a12", "a22", "kappa", "gamma1", "gamma2", "mu")
+
+
+class LhError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"liblh error {code}: {msg}")
+        self.code = code
+
+
+class lh_grid(C.Structure):
+    _fields_ = [("x0", C.c_double), ("y0", C.c_double), ("dx", C.c_double), ("nx", C.c_int32), ("ny", C.c_int32)]
+
+
+class lh_outputs(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in PLANES]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if not os.path.exists(path):
+            raise ImportError(
+                f"{path} is missing: build it with `python -m paper_2004_06352_b200._build` "
+                "(or __graft_entry__.build()). There is no CPU fallback."
+            )
+        L = C.CDLL(path)
+        vp, ci, dp = C.c_void_p, C.c_int, C.c_void_p
+        gp = C.POINTER(lh_grid)
+        op = C.POINTER(lh_outputs)
+        L.lh_grid_gradient.argtypes = [vp, ci, gp, dp, dp]
+        L.lh_grid_hessian.argtypes = [vp, ci, gp, dp, dp, dp]
+        L.lh_lens_maps.argtypes = [vp, ci, gp, dp, dp, dp, dp]
+        L.lh_grid_gradient_batch.argtypes = [vp, ci, ci, gp, dp, dp]
+        L.lh_grid_eval.argtypes = [vp, ci, gp, op]
+        L.lh_grid_eval_batch.argtypes = [vp, ci, ci, gp, op]
+        L.lh_grid_eval_host.argtypes = [vp, ci, ci, gp, op]
+        L.lh_set_stream.argtypes = [vp]
+        L.lh_pack_model.argtypes = [vp, ci, vp, vp]
+        L.lh_pack_model.restype = ci
+        L.lh_last_error.restype = C.c_char_p
+        L.lh_launch_count.restype = C.c_longlong
+        L.lh_fp64_peak_probe.argtypes = [ci, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.lh_version.restype = C.c_char_p
+        for f in ("lh_grid_gradient", "lh_grid_hessian", "lh_lens_maps", "lh_grid_gradient_batch", "lh_grid_eval",
+                  "lh_grid_eval_batch", "lh_grid_eval_host", "lh_set_stream", "lh_fp64_peak_probe"):
+            getattr(L, f).restype = ci
+        _lib = L
+    return _lib
+
+
+# ---------------------------------------------------------------- marshalling helpers
+def _lenses_ptr(lenses):
+    """numpy array of 64-byte lh_lens records (any dtype of itemsize 64), host memory."""
+    a = np.ascontiguousarray(lenses)
+    if a.dtype.itemsize != 64:
+        raise TypeError("lenses must be an array of 64-byte lh_lens records")
+    return a, a.ctypes.data, a.size
+
+
+def _grid(g) -> lh_grid:
+    if isinstance(g, lh_grid):
+        return g
+    return lh_grid(float(g.x0), float(g.y0), float(g.dx), int(g.nx), int(g.ny))
+
+
+def _dev_ptr(t):
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        if hasattr(t, "is_contiguous") and not t.is_contiguous():
+            raise TypeError("output tensors must be contiguous")
+        if hasattr(t, "dtype") and "float64" not in str(t.dtype):
+            raise TypeError("output tensors must be float64")
+        return t.data_ptr()
+    raise TypeError(f"cannot take a device pointer from {type(t)}")
+
+
+def _check(rc: int):
+    if rc != LH_OK:
+        raise LhError(rc, _load().lh_last_error().decode())
+
+
+def _outputs(planes: dict, to_ptr) -> lh_outputs:
+    bad = set(planes) - set(PLANES)
+    if bad:
+        raise KeyError(f"unknown planes {sorted(bad)}")
+    return lh_outputs(**{n: to_ptr(planes.get(n)) for n in PLANES})
+
+
+# ---------------------------------------------------------------- the C ABI, name for name
+def lh_grid_gradient(lenses, grid, out_ax, out_ay):
+    a, p, n = _lenses_ptr(lenses)
+    _check(_load().lh_grid_gradient(p, n, C.byref(_grid(grid)), _dev_ptr(out_ax), _dev_ptr(out_ay)))
+
+
+def lh_grid_hessian(lenses, grid, a11, a12, a22):
+    a, p, n = _lenses_ptr(lenses)
+    _check(_load().lh_grid_hessian(p, n, C.byref(_grid(grid)), _dev_ptr(a11), _dev_ptr(a12), _dev_ptr(a22)))
+
+
+def lh_lens_maps(lenses, grid, kappa, gamma1, gamma2, mu):
+    a, p, n = _lenses_ptr(lenses)
+    _check(_load().lh_lens_maps(p, n, C.byref(_grid(grid)), _dev_ptr(kappa), _dev_ptr(gamma1), _dev_ptr(gamma2),
+                                _dev_ptr(mu)))
+
+
+def lh_grid_gradient_batch(lenses, nmodel, nlens, grid, out_ax, out_ay):
+    a, p, n = _lenses_ptr(lenses)
+    if n != nmodel * nlens:
+        raise ValueError("len(lenses) != nmodel*nlens")
+    _check(_load().lh_grid_gradient_batch(p, nmodel, nlens, C.byref(_grid(grid)), _dev_ptr(out_ax), _dev_ptr(out_ay)))
+
+
+def lh_grid_eval(lenses, grid, **planes):
+    """planes: any of ax, ay, a11, a12, a22, kappa, gamma1, gamma2, mu = device tensor."""
+    a, p, n = _lenses_ptr(lenses)
+    o = _outputs(planes, _dev_ptr)
+    _check(_load().lh_grid_eval(p, n, C.byref(_grid(grid)), C.byref(o)))
+
+
+def lh_grid_eval_batch(lenses, nmodel, nlens, grid, **planes):
+    a, p, n = _lenses_ptr(lenses)
+    if n != nmodel * nlens:
+        raise ValueError("len(lenses) != nmodel*nlens")
+    o = _outputs(planes, _dev_ptr)
+    _check(_load().lh_grid_eval_batch(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(o)))
+
+
+def lh_grid_eval_host(lenses, nmodel, nlens, grid, **host_planes):
+    """host_planes: numpy float64 C-contiguous arrays of nmodel*ny*nx elements (HOST memory,
+    pinned or not); the copies back and a stream synchronise happen inside the call."""
+    a, p, n = _lenses_ptr(lenses)
+    if n != nmodel * nlens:
+        raise ValueError("len(lenses) != nmodel*nlens")
+
+    def host_ptr(v):
+        if v is None:
+            return None
+        if isinstance(v, np.ndarray):
+            if v.dtype != np.float64 or not v.flags.c_contiguous:
+                raise TypeError("host planes must be C-contiguous float64")
+            return v.ctypes.data
+        if hasattr(v, "data_ptr"):  # e.g. a pinned torch CPU tensor
+            return v.data_ptr()
+        raise TypeError(f"cannot take a host pointer from {type(v)}")
+
+    o = _outputs(host_planes, host_ptr)
+    _check(_load().lh_grid_eval_host(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(o)))
+
+
+LH_PACK_DOUBLES, LH_PACK_CLASSES = 28, 3
+
+
+def lh_pack_model(lenses, validate_only: bool = False):
+    """Step a1 on the host: returns (table[n, LH_PACK_DOUBLES], class_begin[LH_PACK_CLASSES+1])."""
+    a, p, n = _lenses_ptr(lenses)
+    begin = np.zeros(LH_PACK_CLASSES + 1, dtype=np.int32)
+    if validate_only:
+        _check(_load().lh_pack_model(p, n, None, begin.ctypes.data))
+        return None, begin
+    raw = np.zeros(n * LH_PACK_DOUBLES + 2, dtype=np.float64)
+    off = (16 - raw.ctypes.data % 16) % 16 // 8
+    table = raw[off: off + n * LH_PACK_DOUBLES]
+    _check(_load().lh_pack_model(p, n, table.ctypes.data, begin.ctypes.data))
+    return table.reshape(n, LH_PACK_DOUBLES), begin
+
+
+def lh_set_stream(stream) -> None:
+    """stream: None (legacy default), an int handle, or a torch.cuda.Stream."""
+    h = 0 if stream is None else (stream if isinstance(stream, int) else stream.cuda_stream)
+    _check(_load().lh_set_stream(h))
+
+
+def lh_last_error() -> str:
+    return _load().lh_last_error().decode()
+
+
+def lh_launch_count() -> int:
+    return int(_load().lh_launch_count())
+
+
+def lh_fp64_peak_probe(iters: int = 4096):
+    f, s = C.c_double(), C.c_double()
+    _check(_load().lh_fp64_peak_probe(int(iters), C.byref(f), C.byref(s)))
+    return f.value, s.value
+
+
+def lh_version() -> str:
+    return _load().lh_version().decode()

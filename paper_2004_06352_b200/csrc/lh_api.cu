@@ -1,0 +1,306 @@
+// lh_api.cu -- the C ABI of liblh.so (include/lh.h): argument checks, host packing,
+// staging of the packed table, launch.  No arithmetic of the method lives here.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/lh.h"
+#include "lh_kernels.h"
+
+namespace {
+
+using lh::EvalParams;
+using lh::LensK;
+using lh::ModelRanges;
+
+// Per-host-thread state: stream, last error, and the staging buffers for the packed
+// table.  The pinned staging area may only be rewritten once the previous H2D copy has
+// finished (ev_copied); the device table may only be overwritten once the previous
+// kernel has finished reading it, which stream order guarantees on one stream and
+// ev_done + cudaStreamWaitEvent guarantees across a stream change.
+struct Context {
+    cudaStream_t stream = nullptr;
+    char err[512] = {0};
+    long long launches = 0;
+
+    void *h_stage = nullptr;  // pinned: [ranges | table]
+    void *d_stage = nullptr;
+    size_t stage_bytes = 0;
+    cudaEvent_t ev_copied = nullptr, ev_done = nullptr;
+    cudaStream_t last_stream = nullptr;
+    bool busy = false;
+
+    double *d_planes = nullptr;  // cached device planes for the *_host entry point
+    size_t planes_bytes = 0;
+    double *d_sink = nullptr;
+
+    ~Context() {
+        // process teardown: the CUDA runtime may already be gone; leak deliberately.
+    }
+};
+
+thread_local Context ctx;
+
+int fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    std::vsnprintf(ctx.err, sizeof(ctx.err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) return fail(LH_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));     \
+    } while (0)
+
+const int NPLANES = 9;
+
+void planes_of(const lh_outputs *o, double *p[NPLANES]) {
+    p[0] = o->ax; p[1] = o->ay; p[2] = o->a11; p[3] = o->a12; p[4] = o->a22;
+    p[5] = o->kappa; p[6] = o->gamma1; p[7] = o->gamma2; p[8] = o->mu;
+}
+
+int check_grid(const lh_grid *g, int nmodel) {
+    if (!g) return fail(LH_EINVAL, "grid is NULL");
+    if (g->nx <= 0 || g->ny <= 0) return fail(LH_EINVAL, "grid: nx and ny must be > 0");
+    if (!(std::isfinite(g->x0) && std::isfinite(g->y0) && std::isfinite(g->dx)) || !(g->dx > 0.0))
+        return fail(LH_EINVAL, "grid: x0, y0 must be finite and dx > 0");
+    const long double tot = (long double)g->nx * g->ny * nmodel;
+    if (tot >= (long double)(1ULL << 40)) return fail(LH_EINVAL, "grid: nmodel*nx*ny must be < 2^40");
+    return LH_OK;
+}
+
+int check_device_ptr(const double *p, const char *name) {
+    if ((reinterpret_cast<uintptr_t>(p) & 7u) != 0) return fail(LH_EINVAL, "output %s is not 8-byte aligned", name);
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(LH_EINVAL, "output %s is not a device pointer", name);
+    }
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+        return fail(LH_EINVAL, "output %s is not a device pointer", name);
+    return LH_OK;
+}
+
+const char *PLANE_NAMES[NPLANES] = {"ax", "ay", "a11", "a12", "a22", "kappa", "gamma1", "gamma2", "mu"};
+
+// Validate + pack + stage + launch.  `dev_out` are device planes (already checked).
+int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *dev_out[NPLANES]) {
+    const size_t n_total = (size_t)nmodel * (size_t)nlens;
+    const size_t ranges_bytes = ((size_t)nmodel * sizeof(ModelRanges) + 15) & ~size_t(15);
+    const size_t need = ranges_bytes + n_total * sizeof(LensK);
+
+    if (!ctx.ev_copied) {
+        CU(cudaEventCreateWithFlags(&ctx.ev_copied, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&ctx.ev_done, cudaEventDisableTiming));
+    }
+    if (ctx.busy) CU(cudaEventSynchronize(ctx.ev_copied));  // staging area free again
+    if (need > ctx.stage_bytes) {
+        if (ctx.busy) CU(cudaEventSynchronize(ctx.ev_done));  // old device table no longer read
+        if (ctx.h_stage) cudaFreeHost(ctx.h_stage);
+        if (ctx.d_stage) cudaFree(ctx.d_stage);
+        ctx.h_stage = ctx.d_stage = nullptr;
+        ctx.stage_bytes = 0;
+        const size_t cap = need + need / 2 + 4096;
+        CU(cudaMallocHost(&ctx.h_stage, cap));
+        CU(cudaMalloc(&ctx.d_stage, cap));
+        ctx.stage_bytes = cap;
+    }
+
+    // a1: pack on the host straight into the pinned staging area
+    ModelRanges *h_ranges = static_cast<ModelRanges *>(ctx.h_stage);
+    LensK *h_table = reinterpret_cast<LensK *>(static_cast<char *>(ctx.h_stage) + ranges_bytes);
+    for (int m = 0; m < nmodel; ++m) {
+        if (lh::pack_model(lenses + (size_t)m * nlens, nlens, h_table + (size_t)m * nlens, h_ranges + m, ctx.err,
+                           sizeof(ctx.err), m) != 0)
+            return LH_EINVAL;  // message already written; nothing enqueued
+    }
+
+    cudaStream_t s = ctx.stream;
+    if (ctx.busy && ctx.last_stream != s) CU(cudaStreamWaitEvent(s, ctx.ev_done, 0));
+    CU(cudaMemcpyAsync(ctx.d_stage, ctx.h_stage, need, cudaMemcpyHostToDevice, s));
+    CU(cudaEventRecord(ctx.ev_copied, s));
+
+    EvalParams P;
+    P.ranges = static_cast<const ModelRanges *>(ctx.d_stage);
+    P.table = reinterpret_cast<const LensK *>(static_cast<char *>(ctx.d_stage) + ranges_bytes);
+    P.nlens = nlens;
+    P.nmodel = nmodel;
+    P.x0 = g->x0; P.y0 = g->y0; P.dx = g->dx;
+    P.nx = g->nx; P.ny = g->ny;
+    P.plane = (long long)g->nx * g->ny;
+    for (int k = 0; k < NPLANES; ++k) P.out[k] = dev_out[k];
+    P.tiles_x = P.tiles_y = 0;
+    CU(lh::launch_eval(P, s));
+    ++ctx.launches;
+    CU(cudaEventRecord(ctx.ev_done, s));
+    ctx.busy = true;
+    ctx.last_stream = s;
+    return LH_OK;
+}
+
+int check_common(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g) {
+    if (nmodel < 1) return fail(LH_EINVAL, "nmodel must be >= 1");
+    if (nlens < 0) return fail(LH_EINVAL, "nlens must be >= 0");
+    if (nlens > 0 && !lenses) return fail(LH_EINVAL, "lenses is NULL");
+    if ((long double)nmodel * nlens >= (long double)(1u << 30)) return fail(LH_EINVAL, "nmodel*nlens must be < 2^30");
+    return check_grid(g, nmodel);
+}
+
+int eval_checked(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *o) {
+    ctx.err[0] = 0;
+    int rc = check_common(lenses, nmodel, nlens, g);
+    if (rc) return rc;
+    if (!o) return fail(LH_EINVAL, "outputs is NULL");
+    double *p[NPLANES];
+    planes_of(o, p);
+    bool any = false;
+    for (int k = 0; k < NPLANES; ++k) {
+        if (!p[k]) continue;
+        any = true;
+        if ((rc = check_device_ptr(p[k], PLANE_NAMES[k]))) return rc;
+    }
+    if (!any) return fail(LH_EINVAL, "no output plane requested");
+    return eval_device(lenses, nmodel, nlens, g, p);
+}
+
+}  // namespace
+
+extern "C" {
+
+int lh_grid_eval(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_outputs *o) {
+    return eval_checked(lenses, 1, nlens, g, o);
+}
+
+int lh_grid_eval_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *o) {
+    return eval_checked(lenses, nmodel, nlens, g, o);
+}
+
+int lh_grid_gradient(const lh_lens *lenses, int nlens, const lh_grid *g, double *out_ax, double *out_ay) {
+    if (!out_ax || !out_ay) return fail(LH_EINVAL, "lh_grid_gradient: out_ax and out_ay are required");
+    lh_outputs o;
+    std::memset(&o, 0, sizeof(o));
+    o.ax = out_ax; o.ay = out_ay;
+    return eval_checked(lenses, 1, nlens, g, &o);
+}
+
+int lh_grid_hessian(const lh_lens *lenses, int nlens, const lh_grid *g, double *a11, double *a12, double *a22) {
+    if (!a11 || !a12 || !a22) return fail(LH_EINVAL, "lh_grid_hessian: a11, a12 and a22 are required");
+    lh_outputs o;
+    std::memset(&o, 0, sizeof(o));
+    o.a11 = a11; o.a12 = a12; o.a22 = a22;
+    return eval_checked(lenses, 1, nlens, g, &o);
+}
+
+int lh_lens_maps(const lh_lens *lenses, int nlens, const lh_grid *g, double *kappa, double *gamma1, double *gamma2,
+                 double *mu) {
+    if (!kappa || !gamma1 || !gamma2 || !mu) return fail(LH_EINVAL, "lh_lens_maps: all four planes are required");
+    lh_outputs o;
+    std::memset(&o, 0, sizeof(o));
+    o.kappa = kappa; o.gamma1 = gamma1; o.gamma2 = gamma2; o.mu = mu;
+    return eval_checked(lenses, 1, nlens, g, &o);
+}
+
+int lh_grid_gradient_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *out_ax,
+                           double *out_ay) {
+    if (!out_ax || !out_ay) return fail(LH_EINVAL, "lh_grid_gradient_batch: out_ax and out_ay are required");
+    lh_outputs o;
+    std::memset(&o, 0, sizeof(o));
+    o.ax = out_ax; o.ay = out_ay;
+    return eval_checked(lenses, nmodel, nlens, g, &o);
+}
+
+int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *host_o) {
+    ctx.err[0] = 0;
+    int rc = check_common(lenses, nmodel, nlens, g);
+    if (rc) return rc;
+    if (!host_o) return fail(LH_EINVAL, "outputs is NULL");
+    double *hp[NPLANES], *dp[NPLANES];
+    planes_of(host_o, hp);
+    int nreq = 0;
+    for (int k = 0; k < NPLANES; ++k) nreq += hp[k] != nullptr;
+    if (!nreq) return fail(LH_EINVAL, "no output plane requested");
+    const size_t plane_bytes = (size_t)nmodel * g->nx * g->ny * sizeof(double);
+    const size_t need = plane_bytes * nreq;
+    if (need > ctx.planes_bytes) {
+        if (ctx.d_planes) {
+            CU(cudaStreamSynchronize(ctx.stream));
+            cudaFree(ctx.d_planes);
+            ctx.d_planes = nullptr;
+            ctx.planes_bytes = 0;
+        }
+        CU(cudaMalloc(&ctx.d_planes, need));
+        ctx.planes_bytes = need;
+    }
+    int slot = 0;
+    for (int k = 0; k < NPLANES; ++k)
+        dp[k] = hp[k] ? ctx.d_planes + (size_t)(slot++) * (plane_bytes / sizeof(double)) : nullptr;
+    rc = eval_device(lenses, nmodel, nlens, g, dp);
+    if (rc) return rc;
+    for (int k = 0; k < NPLANES; ++k)
+        if (hp[k]) CU(cudaMemcpyAsync(hp[k], dp[k], plane_bytes, cudaMemcpyDeviceToHost, ctx.stream));
+    CU(cudaStreamSynchronize(ctx.stream));
+    return LH_OK;
+}
+
+int lh_pack_model(const lh_lens *lenses, int n, double *table, int32_t *class_begin) {
+    static_assert(LH_PACK_DOUBLES == lh::LENSK_DOUBLES && LH_PACK_CLASSES == lh::CLS_COUNT, "lh.h out of date");
+    ctx.err[0] = 0;
+    if (n < 0 || (n > 0 && !lenses) || !class_begin) return fail(LH_EINVAL, "lh_pack_model: bad argument");
+    LensK *tmp = table ? reinterpret_cast<LensK *>(table) : new (std::nothrow) LensK[n > 0 ? n : 1];
+    if (!tmp) return fail(LH_EINVAL, "lh_pack_model: out of memory");
+    if (table && (reinterpret_cast<uintptr_t>(table) & 15u)) return fail(LH_EINVAL, "table must be 16-byte aligned");
+    ModelRanges r;
+    const int rc = lh::pack_model(lenses, n, tmp, &r, ctx.err, sizeof(ctx.err), 0);
+    if (!table) delete[] tmp;
+    if (rc != 0) return LH_EINVAL;
+    for (int k = 0; k <= lh::CLS_COUNT; ++k) class_begin[k] = r.begin[k];
+    return LH_OK;
+}
+
+int lh_set_stream(void *cuda_stream) {
+    ctx.stream = static_cast<cudaStream_t>(cuda_stream);
+    return LH_OK;
+}
+
+const char *lh_last_error(void) { return ctx.err; }
+
+long long lh_launch_count(void) { return ctx.launches; }
+
+int lh_fp64_peak_probe(int iters, double *flops_per_s, double *seconds) {
+    ctx.err[0] = 0;
+    if (iters <= 0 || !flops_per_s || !seconds) return fail(LH_EINVAL, "lh_fp64_peak_probe: bad argument");
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (!ctx.d_sink) CU(cudaMalloc(&ctx.d_sink, 64));
+    const int blocks = sms * 8;  // 8 x 256 threads = 64 warps per SM
+    cudaEvent_t t0, t1;
+    CU(cudaEventCreate(&t0));
+    CU(cudaEventCreate(&t1));
+    CU(lh::launch_dfma_probe(iters / 8 + 1, blocks, ctx.d_sink, ctx.stream));  // warm-up
+    CU(cudaEventRecord(t0, ctx.stream));
+    CU(lh::launch_dfma_probe(iters, blocks, ctx.d_sink, ctx.stream));
+    CU(cudaEventRecord(t1, ctx.stream));
+    CU(cudaEventSynchronize(t1));
+    ctx.launches += 2;
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, t0, t1));
+    cudaEventDestroy(t0);
+    cudaEventDestroy(t1);
+    const double fmas = (double)blocks * 256.0 * (double)iters * 64.0;
+    *seconds = ms * 1e-3;
+    *flops_per_s = 2.0 * fmas / (*seconds);
+    return LH_OK;
+}
+
+const char *lh_version(void) { return "lh 0.1 sm_100a"; }
+
+}  // extern "C"

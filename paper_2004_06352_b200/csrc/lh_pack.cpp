@@ -1,0 +1,108 @@
+// lh_pack.cpp -- host side of step a1: validate the boundary AoS and precompute the
+// per-lens constants (O(nlens), double precision, plain C++; no CUDA in here).
+#include "lh_pack.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "../../include/lh.h"
+
+namespace lh {
+
+static bool finite_all(const lh_lens &L) {
+    return std::isfinite(L.x) && std::isfinite(L.y) && std::isfinite(L.ellipticity) && std::isfinite(L.theta) &&
+           std::isfinite(L.rcore) && std::isfinite(L.rcut) && std::isfinite(L.b0);
+}
+
+static int classify(const lh_lens &L, int idx, int model, char *err, int errlen) {
+    auto fail = [&](const char *why) {
+        std::snprintf(err, errlen, "lens %d of model %d: %s", idx, model, why);
+        return -1;
+    };
+    if (L.type != LH_DPIE && L.type != LH_NSIE && L.type != LH_SIS) return fail("unknown type");
+    if (L.type == LH_SIS) {
+        // ellipticity, theta, rcore, rcut are ignored for an SIS (reading 8c-19) -- only what is used must be finite
+        if (!(std::isfinite(L.x) && std::isfinite(L.y) && std::isfinite(L.b0))) return fail("non-finite parameter");
+        return CLS_SIS;
+    }
+    if (L.type == LH_NSIE) {
+        if (!(std::isfinite(L.x) && std::isfinite(L.y) && std::isfinite(L.ellipticity) && std::isfinite(L.theta) &&
+              std::isfinite(L.rcore) && std::isfinite(L.b0)))
+            return fail("non-finite parameter");
+    } else if (!finite_all(L)) {
+        return fail("non-finite parameter");
+    }
+    if (!(L.ellipticity >= 0.0 && L.ellipticity < 1.0)) return fail("ellipticity outside [0,1)");
+    if (!(L.rcore > 0.0)) return fail("rcore must be > 0");
+    if (L.type == LH_DPIE && !(L.rcut > L.rcore)) return fail("dPIE needs rcut > rcore");
+    return L.type == LH_DPIE ? CLS_DPIE : CLS_NSIE;
+}
+
+static void fill(const lh_lens &L, int cls, LensK &K) {
+    std::memset(&K, 0, sizeof(K));
+    K.xc = L.x;
+    K.yc = L.y;
+    if (cls == CLS_SIS) {
+        K.T = L.b0;
+        K.c = 1.0;
+        return;
+    }
+    const double e = L.ellipticity;
+    const double eps = e / (1.0 + std::sqrt(1.0 - e * e));  // reading 8c-2
+    const double o = 1.0 - eps * eps, p = (1.0 + eps) * (1.0 + eps), m = (1.0 - eps) * (1.0 - eps);
+    const double rc = L.rcore;
+    const bool cut = (cls == CLS_DPIE);
+    const double rt = cut ? L.rcut : 0.0;
+    const double T = cut ? L.b0 * rt / (rt - rc) : L.b0;
+    const double c2 = std::cos(2.0 * L.theta), s2 = std::sin(2.0 * L.theta);
+    K.c = std::cos(L.theta);
+    K.s = std::sin(L.theta);
+    K.ip = 1.0 / p;
+    K.im = 1.0 / m;
+    K.rc2 = rc * rc;
+    K.rt2 = rt * rt;
+    K.o = o;
+    K.e4 = 4.0 * eps;
+    K.prc = p * rc;
+    K.prt = p * rt;
+    K.mrc = m * rc;
+    K.mrt = m * rt;
+    K.pdr = p * (rt - rc);
+    K.mdr = m * (rt - rc);
+    K.se = 2.0 * std::sqrt(eps);
+    K.To = T * o;
+    K.T = T;
+    K.orc2 = 2.0 * o * rc;
+    K.ort2 = 2.0 * o * rt;
+    K.c0c = 2.0 * (1.0 + eps * eps) * rc * rc;
+    K.c0t = 2.0 * (1.0 + eps * eps) * rt * rt;
+    K.kdc = -4.0 * eps * c2 * rc * rc;
+    K.kdt = -4.0 * eps * c2 * rt * rt;
+    K.k12c = -2.0 * eps * s2 * rc * rc;
+    K.k12t = -2.0 * eps * s2 * rt * rt;
+}
+
+int pack_model(const void *records, int n, LensK *out, ModelRanges *ranges, char *err, int errlen, int model) {
+    const lh_lens *L = static_cast<const lh_lens *>(records);
+    int count[CLS_COUNT] = {0, 0, 0};
+    // pass 1: validate + count (stable counting sort keeps index order inside a class)
+    for (int i = 0; i < n; ++i) {
+        int cls = classify(L[i], i, model, err, errlen);
+        if (cls < 0) return -1;
+        ++count[cls];
+    }
+    int pos[CLS_COUNT];
+    ranges->begin[0] = 0;
+    for (int k = 0; k < CLS_COUNT; ++k) {
+        pos[k] = ranges->begin[k];
+        ranges->begin[k + 1] = ranges->begin[k] + count[k];
+    }
+    for (int i = 0; i < n; ++i) {
+        int cls = classify(L[i], i, model, err, errlen);
+        fill(L[i], cls, out[pos[cls]++]);
+    }
+    return 0;
+}
+
+}  // namespace lh

@@ -1,0 +1,54 @@
+// lh_pack.h -- device-side lens table produced by the host packer (a1 in DESIGN.md sec. 1).
+//
+// The boundary takes an AoS of raw parameters (lh_lens); the device wants, per
+// lens, the constants that do not depend on the pixel.  PAPER.md:151 (sec. 3.2.1)
+// argues for SoA so that SIMD lanes over *lenses* load homogeneous data; on the
+// GPU the lanes run over *pixels* and every lane of a warp needs the same lens at
+// the same time, so the right layout is one contiguous, 16-byte aligned record
+// per lens that a warp fetches from shared memory as broadcast 128-bit loads.
+#pragma once
+#include <cstdint>
+
+namespace lh {
+
+// Evaluation classes (the table is sorted by class so each inner loop is type-pure).
+enum LensClass : int {
+    CLS_DPIE = 0,  // dPIE, merged one-atan/one-atanh form
+    CLS_NSIE = 1,  // single PIEMD term
+    CLS_SIS = 2,   // singular isothermal sphere
+    CLS_COUNT = 3
+};
+
+// Notation: eps = e/(1+sqrt(1-e^2)), o = 1-eps^2, p = (1+eps)^2,
+// m = (1-eps)^2, T = b0*rt/(rt-rc) (dPIE) or b0 (NSIE, SIS), c/s = cos/sin(theta).
+struct alignas(16) LensK {
+    double xc, yc;      // centre
+    double c, s;        // cos(theta), sin(theta)
+    double ip, im;      // 1/p, 1/m            -> rho^2 = ip x'^2 + im y'^2
+    double rc2, rt2;    // rcore^2, rcut^2     -> w_r^2 = r^2 + rho^2
+    double o, e4;       // 1-eps^2, 4 eps
+    double prc, prt;    // p*rcore, p*rcut     -> P_r = o w_r + p r
+    double mrc, mrt;    // m*rcore, m*rcut     -> Q_r = o w_r + m r
+    double pdr, mdr;    // p*(rt-rc), m*(rt-rc)
+    double se, To;      // 2 sqrt(eps), T*o
+    double T, _r0;      // T
+    double orc2, ort2;  // 2 o rcore, 2 o rcut -> D_r = c0_r + R^2 + (2 o r) w_r
+    double c0c, c0t;    // 2 (1+eps^2) r^2
+    double kdc, kdt;    // -4 eps cos(2 theta) r^2   (N11 - N22 = kd - (dx^2-dy^2))
+    double k12c, k12t;  // -2 eps sin(2 theta) r^2   (N12 = k12 - dx dy)
+};
+static_assert(sizeof(LensK) == 28 * 8, "LensK is 28 doubles");
+constexpr int LENSK_DOUBLES = sizeof(LensK) / 8;
+
+// Per-model class boundaries inside that model's slice of the table:
+// class k occupies [begin[k], begin[k+1]).
+struct ModelRanges {
+    int32_t begin[CLS_COUNT + 1];
+};
+
+// Host: validate `n` boundary records (include/lh.h rules) and fill `out[n]` sorted
+// by class, `ranges` for this model.  Returns 0 or writes a message into err.
+int pack_model(const void *lh_lens_records, int n, LensK *out, ModelRanges *ranges, char *err, int errlen,
+               int model_index);
+
+}  // namespace lh

@@ -1,0 +1,50 @@
+"""Tolerance rules for CUDA-vs-oracle parity (BASELINE.json north_star, readings 8c-13/14).
+
+Plain rule, every plane P:   |d| <= max(1e-11 |P_ref|, 1e-13 max|P_ref|)
+mu (ill-conditioned near critical lines):
+    |d mu| <= 1e-11 |mu_ref| max(1, C),  C = ((1-kappa)^2 + gamma^2) |mu_ref|
+    AND the plain rule on 1/mu.
+"""
+import numpy as np
+
+REL, FLOOR = 1e-11, 1e-13
+
+
+def plain_violation(got, ref):
+    """max over elements of |d| / allowed (<= 1 passes)."""
+    got = np.asarray(got, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    if ref.size == 0:
+        return 0.0
+    allowed = np.maximum(REL * np.abs(ref), FLOOR * np.max(np.abs(ref)))
+    allowed = np.maximum(allowed, 5e-324)
+    d = np.abs(got - ref)
+    d = np.where((got == ref), 0.0, d)  # equal infinities / zeros
+    return float(np.max(d / allowed))
+
+
+def mu_violation(mu_got, mu_ref, kappa_ref, g1_ref, g2_ref):
+    mu_got = np.asarray(mu_got, dtype=np.float64)
+    mu_ref = np.asarray(mu_ref, dtype=np.float64)
+    C = ((1.0 - kappa_ref) ** 2 + g1_ref ** 2 + g2_ref ** 2) * np.abs(mu_ref)
+    allowed = REL * np.abs(mu_ref) * np.maximum(1.0, C)
+    fin = np.isfinite(mu_ref)
+    v1 = float(np.max(np.abs(mu_got - mu_ref)[fin] / allowed[fin])) if fin.any() else 0.0
+    assert np.array_equal(mu_got[~fin], mu_ref[~fin])
+    with np.errstate(divide="ignore"):
+        v2 = plain_violation(1.0 / mu_got, 1.0 / mu_ref)
+    return max(v1, v2)
+
+
+def check_planes(got: dict, ref: dict, what=""):
+    """got/ref: name -> array. ref must hold kappa, gamma1, gamma2 when mu is compared."""
+    worst = {}
+    for n in got:
+        if n == "mu":
+            v = mu_violation(got["mu"], ref["mu"], ref["kappa"], ref["gamma1"], ref["gamma2"])
+        else:
+            v = plain_violation(got[n], ref[n])
+        worst[n] = v
+    bad = {n: v for n, v in worst.items() if not v <= 1.0}
+    assert not bad, f"{what}: parity violated (|d|/allowed): {bad}"
+    return worst

@@ -1,0 +1,130 @@
+"""CPU-only checks of the boundary: liblh.so loads, exports every symbol include/lh.h
+declares, and the host logic (step a1: validation, class sorting, per-lens constants;
+argument checks that fail before any CUDA work) behaves.  No compute calls here."""
+import ctypes
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+import lens_inputs as li
+import paper_2004_06352_b200 as lh
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "lh.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(lh_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    lh._build.build()
+    lib = ctypes.CDLL(lh.library_path())
+    names = declared_functions()
+    assert {"lh_grid_gradient", "lh_grid_hessian", "lh_lens_maps", "lh_grid_gradient_batch", "lh_grid_eval",
+            "lh_grid_eval_batch", "lh_grid_eval_host", "lh_set_stream", "lh_last_error"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in lh.h but not exported"
+    assert lh.lh_version().endswith("sm_100a")
+
+
+def test_binding_has_the_same_names():
+    for n in declared_functions():
+        assert callable(getattr(lh, n)), n
+
+
+def test_struct_layouts_match_header():
+    assert li.LENS_DTYPE.itemsize == 64
+    assert ctypes.sizeof(lh.lh_grid) == 32 and ctypes.sizeof(lh.lh_outputs) == 72
+    offs = {n: li.LENS_DTYPE.fields[n][1] for n in li.LENS_DTYPE.names}
+    assert offs == {"type": 0, "_pad": 4, "x": 8, "y": 16, "ellipticity": 24, "theta": 32, "rcore": 40,
+                    "rcut": 48, "b0": 56}
+
+
+def test_pack_sorts_by_class_and_is_stable():
+    c = li.config(2)
+    table, begin = lh.lh_pack_model(c.lenses)
+    assert list(begin) == [0, 402, 451, 500]
+    for cls, t in ((0, li.DPIE), (1, li.NSIE), (2, li.SIS)):
+        src = c.lenses[c.lenses["type"] == t]
+        sl = table[begin[cls]:begin[cls + 1]]
+        assert np.array_equal(sl[:, 0], src["x"]) and np.array_equal(sl[:, 1], src["y"])  # index order kept
+
+
+def test_pack_constants():
+    """Per-lens constants: recomputed here from their definitions."""
+    L = li.lens(li.DPIE, 1.5, -2.0, 0.6, 0.3, 0.25, 40.0, 3.0)
+    t, _ = lh.lh_pack_model(L)
+    k = t[0]
+    eps = 1.0 / 3.0  # e-hat 0.6 <-> eps 1/3 (reading 8c-2)
+    o, p, m = 1 - eps ** 2, (1 + eps) ** 2, (1 - eps) ** 2
+    T = 3.0 * 40.0 / (40.0 - 0.25)
+    want = [1.5, -2.0, math.cos(0.3), math.sin(0.3), 1 / p, 1 / m, 0.25 ** 2, 40.0 ** 2, o, 4 * eps, p * 0.25,
+            p * 40.0, m * 0.25, m * 40.0, p * 39.75, m * 39.75, 2 * math.sqrt(eps), T * o, T]
+    assert np.allclose(k[:19], want, rtol=1e-15, atol=0)
+    assert np.allclose(k[20:], [2 * o * 0.25, 2 * o * 40.0, 2 * (1 + eps ** 2) * 0.0625, 2 * (1 + eps ** 2) * 1600,
+                                -4 * eps * math.cos(0.6) * 0.0625, -4 * eps * math.cos(0.6) * 1600,
+                                -2 * eps * math.sin(0.6) * 0.0625, -2 * eps * math.sin(0.6) * 1600], rtol=1e-15)
+
+
+@pytest.mark.parametrize("field,value,ok", [
+    ("type", 7, False), ("ellipticity", 1.0, False), ("ellipticity", -0.1, False), ("ellipticity", 0.0, True),
+    ("rcore", 0.0, False), ("rcut", 0.05, False), ("b0", float("nan"), False), ("x", float("inf"), False),
+    ("theta", float("nan"), False), ("b0", 0.0, True), ("b0", -1.0, True),
+])
+def test_pack_validation(field, value, ok):
+    L = li.lens(li.DPIE, 0.0, 0.0, 0.3, 0.1, 0.1, 10.0, 1.0)
+    L[field][0] = value
+    if ok:
+        lh.lh_pack_model(L, validate_only=True)
+    else:
+        with pytest.raises(lh.LhError) as e:
+            lh.lh_pack_model(L, validate_only=True)
+        assert e.value.code == lh.LH_EINVAL and "lens 0" in str(e.value)
+
+
+def test_sis_and_nsie_ignore_unused_fields():
+    lh.lh_pack_model(li.lens(li.SIS, 0, 0, float("nan"), float("nan"), -1.0, float("nan"), 1.0), validate_only=True)
+    lh.lh_pack_model(li.lens(li.NSIE, 0, 0, 0.2, 0.0, 0.1, float("nan"), 1.0), validate_only=True)
+    with pytest.raises(lh.LhError):
+        lh.lh_pack_model(li.lens(li.NSIE, 0, 0, 0.2, 0.0, 0.0, 1.0, 1.0), validate_only=True)
+
+
+def test_argument_errors_before_any_cuda_work():
+    c = li.config(0)
+    g = c.grid
+    bad_grids = [li.Grid(g.x0, g.y0, 0.0, 8, 8), li.Grid(g.x0, g.y0, g.dx, 0, 8), li.Grid(g.x0, g.y0, g.dx, 8, -1),
+                 li.Grid(float("nan"), g.y0, g.dx, 8, 8), li.Grid(g.x0, g.y0, -1.0, 8, 8),
+                 li.Grid(g.x0, g.y0, g.dx, 2 ** 20, 2 ** 20)]
+    for bg in bad_grids:
+        with pytest.raises(lh.LhError) as e:
+            lh.lh_grid_gradient(c.lenses, bg, 256, 512)
+        assert e.value.code == lh.LH_EINVAL
+    with pytest.raises(lh.LhError) as e:  # NULL output
+        lh.lh_grid_gradient(c.lenses, g, None, 512)
+    assert e.value.code == lh.LH_EINVAL
+    with pytest.raises(lh.LhError) as e:  # nothing requested
+        lh.lh_grid_eval(c.lenses, g)
+    assert e.value.code == lh.LH_EINVAL
+    with pytest.raises(lh.LhError) as e:  # misaligned
+        lh.lh_grid_gradient(c.lenses, g, 260, 512)
+    assert "aligned" in str(e.value)
+    with pytest.raises(lh.LhError) as e:  # host address is not device memory
+        buf = np.zeros(g.npix)
+        lh.lh_grid_gradient(c.lenses, g, buf.ctypes.data, buf.ctypes.data)
+    assert e.value.code == lh.LH_EINVAL
+    with pytest.raises(lh.LhError):
+        lh.lh_grid_gradient_batch(c.lenses[:0], 0, 10, g, 256, 512)
+    assert lh.lh_launch_count() == 0
+
+
+def test_missing_library_fails_loudly(monkeypatch, tmp_path):
+    """No CPU fallback: without liblh.so the binding raises."""
+    monkeypatch.setattr(lh, "_lib", None)
+    monkeypatch.setattr(lh._build, "LIB", str(tmp_path / "nope.so"))
+    with pytest.raises(ImportError):
+        lh.lh_version()

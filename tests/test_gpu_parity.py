@@ -1,0 +1,284 @@
+"""CUDA path vs CPU oracle, element by element, through the C ABI (-m gpu).
+
+Small/medium cases compare whole maps; BASELINE.json's full-size configs are run in the
+launch configuration bench.py times and compared on seeded samples of pixels the oracle
+evaluates one by one.  Tolerances: tests/parity.py (north_star: 1e-11 relative, floor
+1e-13 x max|plane|; mu conditioned, reading 8c-13).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import lens_inputs as li
+import oracle
+import paper_2004_06352_b200 as lh
+from parity import check_planes, plain_violation
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+NTHREADS = max(1, min(16, os.cpu_count() or 1))
+
+
+def dev_planes(names, shape):
+    return {n: torch.full(shape, float("nan"), dtype=torch.float64, device="cuda") for n in names}
+
+
+def run_gpu(lenses, grid, names, nmodel=1, nlens=None):
+    nlens = len(lenses) // nmodel if nlens is None else nlens
+    shape = (nmodel, grid.ny, grid.nx) if nmodel > 1 else (grid.ny, grid.nx)
+    out = dev_planes(names, shape)
+    if nmodel == 1:
+        lh.lh_grid_eval(lenses, grid, **out)
+    else:
+        lh.lh_grid_eval_batch(lenses, nmodel, nlens, grid, **out)
+    torch.cuda.synchronize()
+    return {n: v.cpu().numpy() for n, v in out.items()}
+
+
+def ref_grid(lenses, grid, names):
+    need = set(names)
+    if "mu" in need:
+        need |= {"kappa", "gamma1", "gamma2"}
+    return oracle.grid(lenses, grid.x0, grid.y0, grid.dx, grid.nx, grid.ny, planes=tuple(sorted(need)),
+                       threads=NTHREADS)
+
+
+def ref_samples(lenses, grid, ii, jj, names):
+    need = set(names)
+    if "mu" in need:
+        need |= {"kappa", "gamma1", "gamma2"}
+    return oracle.points(lenses, grid.x0 + ii * grid.dx, grid.y0 + jj * grid.dx, planes=tuple(sorted(need)))
+
+
+# ------------------------------------------------------------------ BASELINE.json configs, whole maps
+def test_cfg0_all_nine_planes_and_the_four_calls():
+    c = li.config(0)
+    g = c.grid
+    ref = ref_grid(c.lenses, g, li.ALL_PLANES)
+    got = run_gpu(c.lenses, g, li.ALL_PLANES)
+    check_planes(got, ref, "cfg0 lh_grid_eval")
+    # the four named calls give bit-identical planes to lh_grid_eval's matching kernel variant
+    o = dev_planes(li.ALL_PLANES, (g.ny, g.nx))
+    lh.lh_grid_gradient(c.lenses, g, o["ax"], o["ay"])
+    lh.lh_grid_hessian(c.lenses, g, o["a11"], o["a12"], o["a22"])
+    lh.lh_lens_maps(c.lenses, g, o["kappa"], o["gamma1"], o["gamma2"], o["mu"])
+    torch.cuda.synchronize()
+    check_planes({n: v.cpu().numpy() for n, v in o.items()}, ref, "cfg0 four calls")
+
+
+@pytest.mark.parametrize("idx,scale", [(1, 4), (2, 8), (3, 16)])
+def test_cfg_scaled_whole_map(idx, scale):
+    """configs 1-3 on a coarser grid of the same extent (same lenses): several tiles, every class."""
+    c = li.config(idx, scale=scale)
+    ref = ref_grid(c.lenses, c.grid, c.outputs)
+    got = run_gpu(c.lenses, c.grid, c.outputs)
+    check_planes(got, ref, c.name)
+
+
+def test_cfg4_scaled_batch_whole_maps():
+    c = li.config(4, scale=16)  # 64 models x 300 lenses on 64 x 64
+    got = run_gpu(c.lenses, c.grid, c.outputs, nmodel=c.nmodel, nlens=c.nlens)
+    for m in range(c.nmodel):
+        ref = ref_grid(c.lenses[m * c.nlens:(m + 1) * c.nlens], c.grid, c.outputs)
+        check_planes({n: got[n][m] for n in got}, ref, f"{c.name} model {m}")
+
+
+# ------------------------------------------------------------------ full size, bench launch configuration, sampled
+@pytest.mark.parametrize("idx", [1, 2, 3])
+def test_cfg_full_size_sampled(idx):
+    c = li.config(idx)
+    got = run_gpu(c.lenses, c.grid, c.outputs)
+    ii, jj = li.random_points(100 + idx, c.grid, 3000)
+    # always include the corners and the last row/column (ragged-tail logic at full size)
+    ii = np.concatenate([ii, [0, c.grid.nx - 1, 0, c.grid.nx - 1]])
+    jj = np.concatenate([jj, [0, 0, c.grid.ny - 1, c.grid.ny - 1]])
+    ref = ref_samples(c.lenses, c.grid, ii, jj, c.outputs)
+    check_planes({n: got[n][jj, ii] for n in got}, ref, c.name + " sampled")
+    for n in got:
+        assert np.isfinite(got[n]).all() or n == "mu"
+        assert not np.isnan(got[n]).any()
+
+
+def test_cfg4_full_size_batch_sampled():
+    c = li.config(4)
+    out = dev_planes(c.outputs, (c.nmodel, c.grid.ny, c.grid.nx))
+    lh.lh_grid_gradient_batch(c.lenses, c.nmodel, c.nlens, c.grid, out["ax"], out["ay"])
+    torch.cuda.synchronize()
+    ii, jj = li.random_points(104, c.grid, 400)
+    it, jt = torch.as_tensor(ii, device="cuda"), torch.as_tensor(jj, device="cuda")
+    for m in range(c.nmodel):
+        ref = ref_samples(c.lenses[m * c.nlens:(m + 1) * c.nlens], c.grid, ii, jj, c.outputs)
+        check_planes({n: out[n][m][jt, it].cpu().numpy() for n in out}, ref, f"{c.name} model {m} sampled")
+    assert not torch.isnan(out["ax"]).any() and not torch.isnan(out["ay"]).any()
+
+
+# ------------------------------------------------------------------ tiling edge cases
+@pytest.mark.parametrize("nx,ny", [(1, 1), (1, 9), (9, 1), (63, 3), (64, 4), (65, 5), (67, 7), (129, 2), (200, 13)])
+def test_ragged_grids(nx, ny):
+    c = li.config(2)
+    L = c.lenses[:130]  # 3 tiles of 64 minus a tail; dPIE + NSIE + SIS
+    g = li.Grid(x0=-20.3, y0=11.7, dx=0.37, nx=nx, ny=ny)
+    ref = ref_grid(L, g, li.ALL_PLANES)
+    got = run_gpu(L, g, li.ALL_PLANES)
+    check_planes(got, ref, f"ragged {nx}x{ny}")
+
+
+@pytest.mark.parametrize("nlens", [0, 1, 63, 64, 65, 128, 129])
+def test_lens_counts_around_tile_size(nlens):
+    c = li.config(3)
+    L = c.lenses[:nlens]
+    g = li.Grid(x0=-30.0, y0=-30.0, dx=0.9, nx=70, ny=9)
+    ref = ref_grid(L, g, li.ALL_PLANES)
+    got = run_gpu(L, g, li.ALL_PLANES)
+    check_planes(got, ref, f"nlens={nlens}")
+    if nlens == 0:
+        for n in got:
+            assert np.all(got[n] == (1.0 if n == "mu" else 0.0))
+
+
+def test_mixed_types_any_order():
+    """The library sorts by class; the sum must equal the oracle's index-order sum within tolerance."""
+    c = li.config(2)
+    rng = np.random.default_rng(77)
+    L = c.lenses[rng.permutation(len(c.lenses))[:200]]
+    g = li.Grid(x0=-50.0, y0=-50.0, dx=1.01, nx=99, ny=33)
+    check_planes(run_gpu(L, g, li.ALL_PLANES), ref_grid(L, g, li.ALL_PLANES), "mixed order")
+    for t in (li.NSIE, li.SIS):  # single-class models
+        Lt = c.lenses[c.lenses["type"] == t]
+        check_planes(run_gpu(Lt, g, li.ALL_PLANES), ref_grid(Lt, g, li.ALL_PLANES), f"only type {t}")
+
+
+# ------------------------------------------------------------------ degenerate cases of the method
+@pytest.mark.parametrize("ehat", [0.0, 1e-14, 1e-12, 1e-9, 1e-6, 1e-3, 0.3, 0.9, 0.99, 0.9999])
+def test_ellipticity_range(ehat):
+    L = li.make_lenses(3)
+    L[0] = (li.DPIE, 0, 0.3, -0.2, ehat, 0.7, 0.08, 30.0, 1.7)
+    L[1] = (li.NSIE, 0, -4.0, 2.0, ehat, 2.4, 0.3, 0.0, 0.6)
+    L[2] = (li.DPIE, 0, 5.0, 5.0, ehat, 1.1, 2.0, 900.0, 9.0)
+    g = li.Grid(x0=-15.0, y0=-15.0, dx=0.31, nx=97, ny=97)
+    check_planes(run_gpu(L, g, li.ALL_PLANES), ref_grid(L, g, li.ALL_PLANES), f"ehat={ehat}")
+
+
+def test_pixel_on_and_next_to_centres():
+    g = li.Grid(x0=-1.0, y0=-1.0, dx=0.25, nx=9, ny=9)  # pixel (4,4) is exactly (0,0)
+    L = li.make_lenses(4)
+    L[0] = (li.SIS, 0, 0.0, 0.0, 0, 0, 0, 0, 0.7)              # exactly on a pixel: zero contribution
+    L[1] = (li.DPIE, 0, 0.25 + 1e-9, 0.5, 0.4, 0.3, 0.01, 8.0, 1.0)  # rcore << dx, pixel 1e-9" from centre
+    L[2] = (li.NSIE, 0, -0.5, -0.25, 0.2, 1.0, 0.02, 0.0, 0.4)  # exactly on a pixel
+    L[3] = (li.DPIE, 0, 0.75, -0.75, 0.0, 0.0, 0.05, 3.0, 0.0)  # b0 = 0
+    got = run_gpu(L, g, li.ALL_PLANES)
+    ref = ref_grid(L, g, li.ALL_PLANES)
+    check_planes(got, ref, "centres")
+    assert not any(np.isnan(v).any() for v in got.values())
+    only_sis = run_gpu(L[:1], g, li.ALL_PLANES)
+    assert only_sis["ax"][4, 4] == 0.0 and only_sis["kappa"][4, 4] == 0.0 and only_sis["mu"][4, 4] == 1.0
+
+
+def test_far_field_and_large_scales():
+    """|x| up to 1e4 arcsec and rcut = 1e6: no overflow/cancellation surprises in the merged forms."""
+    L = li.make_lenses(2)
+    L[0] = (li.DPIE, 0, 10.0, -20.0, 0.5, 0.4, 0.5, 1e6, 30.0)
+    L[1] = (li.DPIE, 0, -3.0, 4.0, 0.6, 2.0, 1e-3, 2e-3, 1.0)  # rcut barely above rcore scale
+    g = li.Grid(x0=-1e4, y0=-1e4, dx=157.3, nx=128, ny=128)
+    check_planes(run_gpu(L, g, li.ALL_PLANES), ref_grid(L, g, li.ALL_PLANES), "far field")
+
+
+# ------------------------------------------------------------------ ABI behaviour on the device
+def test_unrequested_planes_are_never_touched():
+    c = li.config(0)
+    g = c.grid
+    for req in (("ax", "ay"), ("kappa", "mu"), ("a12",), ("ay", "gamma1")):
+        out = dev_planes(li.ALL_PLANES, (g.ny, g.nx))
+        lh.lh_grid_eval(c.lenses, g, **{n: out[n] for n in req})
+        torch.cuda.synchronize()
+        for n in li.ALL_PLANES:
+            if n in req:
+                assert not torch.isnan(out[n]).any()
+            else:
+                assert torch.isnan(out[n]).all()
+
+
+def test_guard_bands_not_overwritten():
+    c = li.config(0)
+    g = li.Grid(x0=-10.0, y0=-10.0, dx=0.3, nx=67, ny=5)
+    pad = 64
+    buf = torch.full((2, g.npix + 2 * pad), 7.25, dtype=torch.float64, device="cuda")
+    ax, ay = buf[0, pad:pad + g.npix], buf[1, pad:pad + g.npix]
+    lh.lh_grid_gradient(c.lenses, g, ax, ay)
+    torch.cuda.synchronize()
+    assert (buf[:, :pad] == 7.25).all() and (buf[:, pad + g.npix:] == 7.25).all()
+    # odd plane offset: 8-byte but not 16-byte aligned outputs are legal
+    ax2, ay2 = buf[0, pad + 1:pad + 1 + g.npix - 1], buf[1, pad + 1:pad + 1 + g.npix - 1]
+    g2 = li.Grid(x0=g.x0, y0=g.y0, dx=g.dx, nx=g.npix - 1, ny=1)
+    lh.lh_grid_gradient(c.lenses, g2, ax2, ay2)
+    torch.cuda.synchronize()
+    ref = ref_grid(c.lenses, g2, ("ax", "ay"))
+    check_planes({"ax": ax2.cpu().numpy().reshape(1, -1), "ay": ay2.cpu().numpy().reshape(1, -1)}, ref, "odd offset")
+
+
+def test_batch_of_one_equals_single_call_bitwise():
+    c = li.config(1, scale=8)
+    a = run_gpu(c.lenses, c.grid, ("ax", "ay"))
+    out = dev_planes(("ax", "ay"), (1, c.grid.ny, c.grid.nx))
+    lh.lh_grid_gradient_batch(c.lenses, 1, c.nlens, c.grid, out["ax"], out["ay"])
+    torch.cuda.synchronize()
+    assert np.array_equal(a["ax"], out["ax"][0].cpu().numpy()) and np.array_equal(a["ay"], out["ay"][0].cpu().numpy())
+
+
+def test_errors_write_nothing():
+    c = li.config(0)
+    g = c.grid
+    out = dev_planes(("ax", "ay"), (g.ny, g.nx))
+    before = lh.lh_launch_count()
+    bad = c.lenses.copy()
+    bad["ellipticity"][3] = 1.0
+    with pytest.raises(lh.LhError) as e:
+        lh.lh_grid_gradient(bad, g, out["ax"], out["ay"])
+    assert e.value.code == lh.LH_EINVAL and "lens 3" in str(e.value)
+    cpu = torch.zeros(g.npix, dtype=torch.float64)
+    with pytest.raises(lh.LhError):
+        lh.lh_grid_gradient(c.lenses, g, cpu, out["ay"])  # host tensor is not device memory
+    torch.cuda.synchronize()
+    assert torch.isnan(out["ax"]).all() and torch.isnan(out["ay"]).all()
+    assert lh.lh_launch_count() == before
+    lh.lh_grid_gradient(c.lenses, g, out["ax"], out["ay"])  # and the library still works afterwards
+    torch.cuda.synchronize()
+    assert not torch.isnan(out["ax"]).any()
+
+
+def test_two_streams_do_not_interfere():
+    c1, c3 = li.config(1, scale=4), li.config(3, scale=16)
+    r1, r3 = ref_grid(c1.lenses, c1.grid, ("ax", "ay")), ref_grid(c3.lenses, c3.grid, ("ax", "ay"))
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    o1 = [dev_planes(("ax", "ay"), (c1.grid.ny, c1.grid.nx)) for _ in range(4)]
+    o3 = [dev_planes(("ax", "ay"), (c3.grid.ny, c3.grid.nx)) for _ in range(4)]
+    torch.cuda.synchronize()
+    try:
+        for k in range(4):
+            lh.lh_set_stream(s1)
+            lh.lh_grid_gradient(c1.lenses, c1.grid, o1[k]["ax"], o1[k]["ay"])
+            lh.lh_set_stream(s2)
+            lh.lh_grid_gradient(c3.lenses, c3.grid, o3[k]["ax"], o3[k]["ay"])
+    finally:
+        lh.lh_set_stream(None)
+    torch.cuda.synchronize()
+    for k in range(4):
+        check_planes({n: v.cpu().numpy() for n, v in o1[k].items()}, r1, "stream 1")
+        check_planes({n: v.cpu().numpy() for n, v in o3[k].items()}, r3, "stream 2")
+
+
+def test_host_entry_point_matches_device_entry_point():
+    c = li.config(2, scale=16)
+    g = c.grid
+    dev = run_gpu(c.lenses, g, li.ALL_PLANES)
+    host = {n: np.full((g.ny, g.nx), np.nan) for n in ("ax", "kappa", "mu")}
+    lh.lh_grid_eval_host(c.lenses, 1, c.nlens, g, **host)
+    for n in host:
+        assert np.array_equal(host[n], dev[n])
+
+
+def test_fp64_probe_runs():
+    flops, secs = lh.lh_fp64_peak_probe(2048)
+    assert secs > 0 and 1e12 < flops < 1e14
