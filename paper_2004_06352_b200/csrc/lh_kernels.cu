@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(THREADS) superpose_kernel(const EvalParams P) 
         // a5: epilogue in registers, then stores of the requested planes only
         if (j < P.ny && i0 < P.nx) {
             const size_t idx = (size_t)model * P.plane + (size_t)j * P.nx + i0;
-            const bool pair = (i0 + 1 < P.nx) && ((idx & 1) == 0);  // 16-byte aligned double2
+            const bool two = (i0 + 1 < P.nx);
             double v[9][PX];
 #pragma unroll
             for (int k = 0; k < PX; ++k) {
@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(THREADS) superpose_kernel(const EvalParams P) 
                 if ((pl < 2 && !GRAD) || (pl >= 2 && !HESS)) continue;
                 double *o = P.out[pl];
                 if (o == nullptr) continue;
-                if (pair) {
+                if (two && (reinterpret_cast<uintptr_t>(o + idx) & 15u) == 0) {  // 16-byte aligned double2
                     *reinterpret_cast<double2 *>(o + idx) = make_double2(v[pl][0], v[pl][1]);
                 } else {
                     o[idx] = v[pl][0];
