@@ -136,7 +136,7 @@ long long lh_launch_count(void);
  * host memory `table`, and the class boundaries into class_begin[0..LH_PACK_CLASSES]
  * (class k = records [class_begin[k], class_begin[k+1])).  `table` may be NULL to
  * validate only.  Returns LH_OK or LH_EINVAL (rules as lh_grid_gradient). */
-#define LH_PACK_DOUBLES 28
+#define LH_PACK_DOUBLES 24
 #define LH_PACK_CLASSES 3
 int lh_pack_model(const lh_lens *lenses, int n, double *table, int32_t *class_begin);
 

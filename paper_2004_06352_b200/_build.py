@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblh.so")
 SOURCES = ["lh_api.cu", "lh_kernels.cu", "lh_pack.cpp"]
-HEADERS = ["lh_kernels.h", "lh_pack.h", os.path.join("..", "..", "include", "lh.h")]
+HEADERS = ["lh_kernels.h", "lh_pack.h", "lh_math.cuh", os.path.join("..", "..", "include", "lh.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",

@@ -6,6 +6,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "../../include/lh.h"
@@ -44,6 +45,25 @@ struct Context {
 };
 
 thread_local Context ctx;
+
+// The atan / atanh reduction tables (lh_math.cuh): one read-only device copy per device,
+// made on first use and kept for the life of the process.
+const lh::MathTables *device_math_tables(int dev, cudaError_t *err) {
+    static std::mutex mu;
+    static const lh::MathTables *cache[64] = {nullptr};
+    std::lock_guard<std::mutex> lock(mu);
+    *err = cudaSuccess;
+    if (dev < 0 || dev >= 64) { *err = cudaErrorInvalidDevice; return nullptr; }
+    if (!cache[dev]) {
+        static lh::MathTables host;
+        lh::fill_math_tables(host);
+        void *d = nullptr;
+        if ((*err = cudaMalloc(&d, sizeof(host))) != cudaSuccess) return nullptr;
+        if ((*err = cudaMemcpy(d, &host, sizeof(host), cudaMemcpyHostToDevice)) != cudaSuccess) { cudaFree(d); return nullptr; }
+        cache[dev] = static_cast<const lh::MathTables *>(d);
+    }
+    return cache[dev];
+}
 
 int fail(int code, const char *fmt, ...) {
     va_list ap;
@@ -128,7 +148,12 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     CU(cudaMemcpyAsync(ctx.d_stage, ctx.h_stage, need, cudaMemcpyHostToDevice, s));
     CU(cudaEventRecord(ctx.ev_copied, s));
 
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    cudaError_t terr;
     EvalParams P;
+    P.math = device_math_tables(dev, &terr);
+    if (!P.math) return fail(LH_ECUDA, "math tables: %s", cudaGetErrorString(terr));
     P.ranges = static_cast<const ModelRanges *>(ctx.d_stage);
     P.table = reinterpret_cast<const LensK *>(static_cast<char *>(ctx.d_stage) + ranges_bytes);
     P.nlens = nlens;

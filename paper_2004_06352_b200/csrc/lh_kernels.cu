@@ -10,7 +10,15 @@
 // The Hessian is carried as trace / difference / off-diagonal because that is what both
 // the per-lens algebra and the epilogue (kappa = S/2, gamma1 = Dl/2,
 // gamma2 = a12; eq. 4, 7-9) want; a11 = (S+Dl)/2 and a22 = (S-Dl)/2 only when asked for.
+//
+// The FP64 pipe is the roofline (one warp instruction per two cycles per scheduler), so
+// the per-lens algebra is written for instruction count: sqrt / reciprocal / atan / atanh
+// come from lh_math.cuh (MUFU seed + one cubic step, table range reduction), the two
+// PIEMD terms of a dPIE share one atan and one atanh, and the Hessian
+// needs no rotation.
 #include <cuda_runtime.h>
+
+#include <cstdint>
 
 #include "lh_kernels.h"
 
@@ -26,79 +34,73 @@ struct Acc {
     double ax, ay, S, Dl, a12;
 };
 
-// atan(u)/u and atanh(u)/u, smooth through u = 0 (Appendix A.2)
-__device__ __forceinline__ double atanc(double u) {
-    const double u2 = u * u;
-    if (u2 < 1e-6) return fma(u2, fma(u2, fma(u2, -1.0 / 7.0, 0.2), -1.0 / 3.0), 1.0);
-    return atan(u) / u;
-}
-__device__ __forceinline__ double atanhc(double u) {
-    const double u2 = u * u;
-    if (u2 < 1e-6) return fma(u2, fma(u2, fma(u2, 1.0 / 7.0, 0.2), 1.0 / 3.0), 1.0);
-    return atanh(u) / u;
-}
+using SmemTables = MathTables;  // the atan / atanh reduction tables, staged per CTA
 
 // ---- dPIE: core term minus cut term, merged ---------------------
+//   x' = c dx + s dy, y' = c dy - s dx, rho^2 = x'^2/p + y'^2/m, w_r = sqrt(r^2 + rho^2)
+//   P_r = o w_r + p r, Q_r = o w_r + m r, g_x = 2 sqrt(eps) x', g_y = 2 sqrt(eps) y'
+//   alpha'_x = G atan ( g_x (P_t - P_c) / (P_c P_t + g_x^2) )
+//   alpha'_y = G atanh( g_y (Q_t - Q_c) / (Q_c Q_t - g_y^2) ),   G = T o / (2 sqrt(eps))
+//   D_r = 2(1+eps^2) r^2 + 2 o r w_r + R^2,  f_r = 1/(w_r D_r)
+//   a11 + a22 += T (1/w_c - 1/w_t)
+//   a11 - a22 += T [ K (f_c rc^2 - f_t rt^2) - (dx^2 - dy^2)(f_c - f_t) ],  K  = -4 eps cos 2theta
+//   a12       += T [ K'(f_c rc^2 - f_t rt^2) -  dx dy       (f_c - f_t) ],  K' = -2 eps sin 2theta
 template <bool GRAD, bool HESS>
-__device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Acc &a) {
+__device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Acc &a, const SmemTables &tb) {
     const double dx = X - L.xc, dy = Y - L.yc;
     const double xp = fma(L.c, dx, L.s * dy);
-    const double yp = fma(L.c, dy, -L.s * dx);
+    const double yp = fma(-L.s, dx, L.c * dy);
     const double xx = xp * xp, yy = yp * yp;
     const double rho2 = fma(L.ip, xx, L.im * yy);
-    const double wc = sqrt(L.rc2 + rho2), wt = sqrt(L.rt2 + rho2);
+    double wc, iwc, wt, iwt;
+    rsqrt_sqrt(L.rc2 + rho2, wc, iwc);
+    rsqrt_sqrt(L.rt2 + rho2, wt, iwt);
     if (GRAD) {
         const double Pc = fma(L.o, wc, L.prc), Pt = fma(L.o, wt, L.prt);
         const double Qc = fma(L.o, wc, L.mrc), Qt = fma(L.o, wt, L.mrt);
-        const double dw = wt - wc;
-        const double dP = fma(L.o, dw, L.pdr), dQ = fma(L.o, dw, L.mdr);
-        // Jx(rc)-Jx(rt) = o A atanc(2 sqrt(eps) A),  A = x' dP / (Pc Pt + 4 eps x'^2)
-        // Jy(rc)-Jy(rt) = o B atanhc(2 sqrt(eps) B), B = y' dQ / (Qc Qt - 4 eps y'^2)
-        const double A = xp * dP / fma(L.e4, xx, Pc * Pt);
-        const double B = yp * dQ / fma(-L.e4, yy, Qc * Qt);
-        const double jx = L.To * A * atanc(L.se * A);
-        const double jy = L.To * B * atanhc(L.se * B);
-        a.ax += L.c * jx - L.s * jy;
-        a.ay += L.s * jx + L.c * jy;
+        const double gx = L.se * xp, gy = L.se * yp;
+        const double at = atan_nd(gx * (Pt - Pc), fma(gx, gx, Pc * Pt), tb.at);
+        const double ah = atanh_nd(gy * (Qt - Qc), fma(-gy, gy, Qc * Qt), tb.ah);
+        a.ax = fma(L.cG, at, fma(-L.sG, ah, a.ax));
+        a.ay = fma(L.sG, at, fma(L.cG, ah, a.ay));
     }
     if (HESS) {
         const double R2 = xx + yy;
-        const double q = fma(dx, dx, -dy * dy), dxy = dx * dy;
-        const double iwc = 1.0 / wc, iwt = 1.0 / wt;
         const double Dc = fma(L.orc2, wc, L.c0c + R2), Dt = fma(L.ort2, wt, L.c0t + R2);
-        const double fc = L.T * iwc / Dc, ft = L.T * iwt / Dt;
-        a.S += L.T * (iwc - iwt);
-        a.Dl += fc * (L.kdc - q) - ft * (L.kdt - q);
-        a.a12 += fc * (L.k12c - dxy) - ft * (L.k12t - dxy);
+        const double fc = iwc * rcp(Dc), ft = iwt * rcp(Dt);
+        const double u = fma(fc, L.rc2, -(ft * L.rt2));
+        const double Tv = L.T * (fc - ft);
+        a.S = fma(L.T, iwc - iwt, a.S);
+        a.Dl = fma(L.KT, u, fma(-fma(dx, dx, -(dy * dy)), Tv, a.Dl));
+        a.a12 = fma(L.K2T, u, fma(-(dx * dy), Tv, a.a12));
     }
 }
 
 // ---- NSIE: one PIEMD term ------------------------------------------------------------------
 template <bool GRAD, bool HESS>
-__device__ __forceinline__ void nsie_term(const LensK &L, double X, double Y, Acc &a) {
+__device__ __forceinline__ void nsie_term(const LensK &L, double X, double Y, Acc &a, const SmemTables &tb) {
     const double dx = X - L.xc, dy = Y - L.yc;
     const double xp = fma(L.c, dx, L.s * dy);
-    const double yp = fma(L.c, dy, -L.s * dx);
+    const double yp = fma(-L.s, dx, L.c * dy);
     const double xx = xp * xp, yy = yp * yp;
     const double rho2 = fma(L.ip, xx, L.im * yy);
-    const double wc = sqrt(L.rc2 + rho2);
+    double wc, iwc;
+    rsqrt_sqrt(L.rc2 + rho2, wc, iwc);
     if (GRAD) {
-        const double A = xp / fma(L.o, wc, L.prc);
-        const double B = yp / fma(L.o, wc, L.mrc);
-        const double jx = L.To * A * atanc(L.se * A);
-        const double jy = L.To * B * atanhc(L.se * B);
-        a.ax += L.c * jx - L.s * jy;
-        a.ay += L.s * jx + L.c * jy;
+        const double at = atan_nd(L.se * xp, fma(L.o, wc, L.prc), tb.at);
+        const double ah = atanh_nd(L.se * yp, fma(L.o, wc, L.mrc), tb.ah);
+        a.ax = fma(L.cG, at, fma(-L.sG, ah, a.ax));
+        a.ay = fma(L.sG, at, fma(L.cG, ah, a.ay));
     }
     if (HESS) {
         const double R2 = xx + yy;
-        const double q = fma(dx, dx, -dy * dy), dxy = dx * dy;
-        const double iwc = 1.0 / wc;
         const double Dc = fma(L.orc2, wc, L.c0c + R2);
-        const double fc = L.T * iwc / Dc;
-        a.S += L.T * iwc;
-        a.Dl += fc * (L.kdc - q);
-        a.a12 += fc * (L.k12c - dxy);
+        const double fc = iwc * rcp(Dc);
+        const double u = fc * L.rc2;
+        const double Tv = L.T * fc;
+        a.S = fma(L.T, iwc, a.S);
+        a.Dl = fma(L.KT, u, fma(-fma(dx, dx, -(dy * dy)), Tv, a.Dl));
+        a.a12 = fma(L.K2T, u, fma(-(dx * dy), Tv, a.a12));
     }
 }
 
@@ -107,7 +109,9 @@ template <bool GRAD, bool HESS>
 __device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc &a) {
     const double dx = X - L.xc, dy = Y - L.yc;
     const double R2 = fma(dx, dx, dy * dy);
-    const double iR = (R2 > 0.0) ? rsqrt(R2) : 0.0;
+    double R, iR;
+    rsqrt_sqrt(R2, R, iR);
+    if (!(R2 > 0.0)) iR = 0.0;
     const double g = L.T * iR;
     if (GRAD) {
         a.ax = fma(g, dx, a.ax);
@@ -116,7 +120,7 @@ __device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc
     if (HESS) {
         const double g3 = g * iR * iR;
         a.S += g;
-        a.Dl = fma(-g3, fma(dx, dx, -dy * dy), a.Dl);
+        a.Dl = fma(-g3, fma(dx, dx, -(dy * dy)), a.Dl);
         a.a12 = fma(-g3, dx * dy, a.a12);
     }
 }
@@ -124,6 +128,14 @@ __device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc
 template <bool GRAD, bool HESS>
 __global__ void __launch_bounds__(THREADS) superpose_kernel(const EvalParams P) {
     __shared__ LensK tile[TL];
+    __shared__ SmemTables tb;
+
+    // reduction tables of atan / atanh: global (L2-resident, 18 KB) -> shared, once per CTA
+    {
+        const double2 *src = reinterpret_cast<const double2 *>(P.math);
+        double2 *dst = reinterpret_cast<double2 *>(&tb);
+        for (int t = threadIdx.x; t < (int)(sizeof(SmemTables) / sizeof(double2)); t += THREADS) dst[t] = __ldg(src + t);
+    }
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tx = blockIdx.x % P.tiles_x, ty = blockIdx.x / P.tiles_x;
@@ -158,11 +170,11 @@ __global__ void __launch_bounds__(THREADS) superpose_kernel(const EvalParams P) 
             const int e1 = min(max(rg.begin[2] - base, 0), n);  // end of NSIE
             for (int l = 0; l < e0; ++l) {
 #pragma unroll
-                for (int k = 0; k < PX; ++k) dpie_term<GRAD, HESS>(tile[l], X[k], Y, acc[k]);
+                for (int k = 0; k < PX; ++k) dpie_term<GRAD, HESS>(tile[l], X[k], Y, acc[k], tb);
             }
             for (int l = e0; l < e1; ++l) {
 #pragma unroll
-                for (int k = 0; k < PX; ++k) nsie_term<GRAD, HESS>(tile[l], X[k], Y, acc[k]);
+                for (int k = 0; k < PX; ++k) nsie_term<GRAD, HESS>(tile[l], X[k], Y, acc[k], tb);
             }
             for (int l = e1; l < n; ++l) {
 #pragma unroll
@@ -199,7 +211,7 @@ __global__ void __launch_bounds__(THREADS) superpose_kernel(const EvalParams P) 
                     *reinterpret_cast<double2 *>(o + idx) = make_double2(v[pl][0], v[pl][1]);
                 } else {
                     o[idx] = v[pl][0];
-                    if (i0 + 1 < P.nx) o[idx + 1] = v[pl][1];
+                    if (two) o[idx + 1] = v[pl][1];
                 }
             }
         }

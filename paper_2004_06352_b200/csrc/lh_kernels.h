@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "lh_math.cuh"
 #include "lh_pack.h"
 
 namespace lh {
@@ -9,6 +10,7 @@ namespace lh {
 struct EvalParams {
     const LensK *table;         // [nmodel][nlens], each model sorted by class
     const ModelRanges *ranges;  // [nmodel]
+    const MathTables *math;     // device copy of the atan / atanh reduction tables
     int nlens, nmodel;
     double x0, y0, dx;
     int nx, ny;

@@ -63,24 +63,24 @@ static void fill(const lh_lens &L, int cls, LensK &K) {
     K.rc2 = rc * rc;
     K.rt2 = rt * rt;
     K.o = o;
-    K.e4 = 4.0 * eps;
+    // The kernel evaluates G * atan(se x' .. ) with G = T o / se; at eps == 0 the limit is taken by a
+    // tiny stand-in (2^-500) for se: atan(u) = u exactly below 1e-8, so G * u is exact and (se x')^2 underflows to 0.
+    const double se = 2.0 * std::sqrt(eps);
+    K.se = (se > 0.0) ? se : 0x1p-500;
+    const double G = T * o / K.se;
     K.prc = p * rc;
     K.prt = p * rt;
     K.mrc = m * rc;
     K.mrt = m * rt;
-    K.pdr = p * (rt - rc);
-    K.mdr = m * (rt - rc);
-    K.se = 2.0 * std::sqrt(eps);
-    K.To = T * o;
+    K.cG = K.c * G;
+    K.sG = K.s * G;
     K.T = T;
     K.orc2 = 2.0 * o * rc;
     K.ort2 = 2.0 * o * rt;
     K.c0c = 2.0 * (1.0 + eps * eps) * rc * rc;
     K.c0t = 2.0 * (1.0 + eps * eps) * rt * rt;
-    K.kdc = -4.0 * eps * c2 * rc * rc;
-    K.kdt = -4.0 * eps * c2 * rt * rt;
-    K.k12c = -2.0 * eps * s2 * rc * rc;
-    K.k12t = -2.0 * eps * s2 * rt * rt;
+    K.KT = -4.0 * eps * c2 * T;
+    K.K2T = -2.0 * eps * s2 * T;
 }
 
 int pack_model(const void *records, int n, LensK *out, ModelRanges *ranges, char *err, int errlen, int model) {

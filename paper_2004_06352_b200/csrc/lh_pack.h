@@ -22,22 +22,20 @@ enum LensClass : int {
 // Notation: eps = e/(1+sqrt(1-e^2)), o = 1-eps^2, p = (1+eps)^2,
 // m = (1-eps)^2, T = b0*rt/(rt-rc) (dPIE) or b0 (NSIE, SIS), c/s = cos/sin(theta).
 struct alignas(16) LensK {
-    double xc, yc;      // centre
-    double c, s;        // cos(theta), sin(theta)
-    double ip, im;      // 1/p, 1/m            -> rho^2 = ip x'^2 + im y'^2
-    double rc2, rt2;    // rcore^2, rcut^2     -> w_r^2 = r^2 + rho^2
-    double o, e4;       // 1-eps^2, 4 eps
-    double prc, prt;    // p*rcore, p*rcut     -> P_r = o w_r + p r
-    double mrc, mrt;    // m*rcore, m*rcut     -> Q_r = o w_r + m r
-    double pdr, mdr;    // p*(rt-rc), m*(rt-rc)
-    double se, To;      // 2 sqrt(eps), T*o
-    double T, _r0;      // T
-    double orc2, ort2;  // 2 o rcore, 2 o rcut -> D_r = c0_r + R^2 + (2 o r) w_r
-    double c0c, c0t;    // 2 (1+eps^2) r^2
-    double kdc, kdt;    // -4 eps cos(2 theta) r^2   (N11 - N22 = kd - (dx^2-dy^2))
-    double k12c, k12t;  // -2 eps sin(2 theta) r^2   (N12 = k12 - dx dy)
+    double xc, yc;      //  0  centre
+    double c, s;        //  2  cos(theta), sin(theta)
+    double ip, im;      //  4  1/p, 1/m              -> rho^2 = ip x'^2 + im y'^2
+    double rc2, rt2;    //  6  rcore^2, rcut^2       -> w_r = sqrt(r^2 + rho^2)
+    double o, se;       //  8  1-eps^2; 2 sqrt(eps), replaced by 2^-500 when eps == 0
+    double prc, prt;    // 10  p*rcore, p*rcut       -> P_r = o w_r + p r
+    double mrc, mrt;    // 12  m*rcore, m*rcut       -> Q_r = o w_r + m r
+    double cG, sG;      // 14  cos, sin(theta) * G,  G = T o / se
+    double T, _r0;      // 16  T
+    double orc2, ort2;  // 18  2 o rcore, 2 o rcut   -> D_r = c0_r + R^2 + (2 o r) w_r
+    double c0c, c0t;    // 20  2 (1+eps^2) r^2
+    double KT, K2T;     // 22  -4 eps cos(2 theta) T, -2 eps sin(2 theta) T
 };
-static_assert(sizeof(LensK) == 28 * 8, "LensK is 28 doubles");
+static_assert(sizeof(LensK) == 24 * 8, "LensK is 24 doubles");
 constexpr int LENSK_DOUBLES = sizeof(LensK) / 8;
 
 // Per-model class boundaries inside that model's slice of the table:
