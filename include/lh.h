@@ -137,7 +137,7 @@ long long lh_launch_count(void);
  * (class k = records [class_begin[k], class_begin[k+1])).  `table` may be NULL to
  * validate only.  Returns LH_OK or LH_EINVAL (rules as lh_grid_gradient). */
 #define LH_PACK_DOUBLES 24
-#define LH_PACK_CLASSES 3
+#define LH_PACK_CLASSES 4
 int lh_pack_model(const lh_lens *lenses, int n, double *table, int32_t *class_begin);
 
 /* Diagnostic: runs a register-resident chain of dependent-free FP64 FMAs on every

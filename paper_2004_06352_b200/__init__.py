@@ -183,7 +183,7 @@ def lh_grid_eval_host(lenses, nmodel, nlens, grid, **host_planes):
     _check(_load().lh_grid_eval_host(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(o)))
 
 
-LH_PACK_DOUBLES, LH_PACK_CLASSES = 24, 3
+LH_PACK_DOUBLES, LH_PACK_CLASSES = 24, 4
 
 
 def lh_pack_model(lenses, validate_only: bool = False):

@@ -137,10 +137,12 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     // a1: pack on the host straight into the pinned staging area
     ModelRanges *h_ranges = static_cast<ModelRanges *>(ctx.h_stage);
     LensK *h_table = reinterpret_cast<LensK *>(static_cast<char *>(ctx.h_stage) + ranges_bytes);
+    bool any_extreme = false;
     for (int m = 0; m < nmodel; ++m) {
         if (lh::pack_model(lenses + (size_t)m * nlens, nlens, h_table + (size_t)m * nlens, h_ranges + m, ctx.err,
                            sizeof(ctx.err), m) != 0)
             return LH_EINVAL;  // message already written; nothing enqueued
+        any_extreme |= h_ranges[m].begin[lh::CLS_EXTREME + 1] > h_ranges[m].begin[lh::CLS_EXTREME];
     }
 
     cudaStream_t s = ctx.stream;
@@ -158,6 +160,7 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     P.table = reinterpret_cast<const LensK *>(static_cast<char *>(ctx.d_stage) + ranges_bytes);
     P.nlens = nlens;
     P.nmodel = nmodel;
+    P.any_extreme = any_extreme ? 1 : 0;
     P.x0 = g->x0; P.y0 = g->y0; P.dx = g->dx;
     P.nx = g->nx; P.ny = g->ny;
     P.plane = (long long)g->nx * g->ny;

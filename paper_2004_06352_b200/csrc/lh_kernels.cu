@@ -24,11 +24,21 @@
 
 namespace lh {
 
-constexpr int PX = 2;              // pixels per thread (adjacent in x -> one double2 store per plane)
-constexpr int TILE_W = 32 * PX;    // one warp spans 64 pixels of a row
-constexpr int TILE_H = 4;          // warps per CTA, one row each
+#ifndef LH_PX
+#define LH_PX 2  // pixels per thread (adjacent in x -> one double2 store per plane)
+#endif
+#ifndef LH_WARPS
+#define LH_WARPS 4  // warps per CTA, one grid row each
+#endif
+#ifndef LH_MINB
+#define LH_MINB 4  // CTAs per SM the register allocation is held to (__launch_bounds__)
+#endif
+constexpr int PX = LH_PX;
+constexpr int TILE_W = 32 * PX;    // one warp spans 32*PX pixels of a row
+constexpr int TILE_H = LH_WARPS;
 constexpr int THREADS = 32 * TILE_H;
 constexpr int TL = 64;             // lenses per shared-memory tile
+static_assert(PX % 2 == 0, "PX must be even (double2 stores)");
 
 struct Acc {
     double ax, ay, S, Dl, a12;
@@ -104,6 +114,52 @@ __device__ __forceinline__ void nsie_term(const LensK &L, double X, double Y, Ac
     }
 }
 
+// ---- CLS_EXTREME: dPIE / NSIE with eps > EXTREME_EPS (axis ratio < 0.02) ----------------------
+// Rare and slow on purpose: the two PIEMD terms are evaluated one by one with
+// IEEE sqrt / division and libdevice atan / atanh -- no table range limits, no merged-form
+// cancellation in d = Q_c Q_t - g_y^2 as u -> 1.  Not inlined: keeps its registers out of the
+// fast loops.  L.rt2 == 0 marks an NSIE (no cut term).
+template <bool GRAD, bool HESS>
+__device__ __forceinline__ void extreme_term(const LensK &L, double X, double Y, Acc &a) {
+    const double dx = X - L.xc, dy = Y - L.yc;
+    const double xp = fma(L.c, dx, L.s * dy);
+    const double yp = fma(-L.s, dx, L.c * dy);
+    const double xx = xp * xp, yy = yp * yp;
+    const double rho2 = fma(L.ip, xx, L.im * yy);
+    const double R2 = xx + yy;
+    const double gx = L.se * xp, gy = L.se * yp;
+    const bool cut = L.rt2 > 0.0;
+    double jx = 0.0, jy = 0.0, S = 0.0, u = 0.0, f = 0.0;
+#pragma unroll 1
+    for (int term = 0; term < 2; ++term) {
+        if (term == 1 && !cut) break;
+        const double r2 = term ? L.rt2 : L.rc2, pr = term ? L.prt : L.prc, mr = term ? L.mrt : L.mrc;
+        const double or2 = term ? L.ort2 : L.orc2, c0 = term ? L.c0t : L.c0c;
+        const double sg = term ? -1.0 : 1.0;
+        const double w = sqrt(r2 + rho2);
+        if (GRAD) {
+            jx += sg * atan(gx / fma(L.o, w, pr));
+            jy += sg * atanh(gy / fma(L.o, w, mr));
+        }
+        if (HESS) {
+            const double fr = 1.0 / (w * fma(or2, w, c0 + R2));
+            S += sg / w;
+            u += sg * fr * r2;
+            f += sg * fr;
+        }
+    }
+    if (GRAD) {
+        a.ax = fma(L.cG, jx, fma(-L.sG, jy, a.ax));
+        a.ay = fma(L.sG, jx, fma(L.cG, jy, a.ay));
+    }
+    if (HESS) {
+        const double Tv = L.T * f;
+        a.S = fma(L.T, S, a.S);
+        a.Dl = fma(L.KT, u, fma(-fma(dx, dx, -(dy * dy)), Tv, a.Dl));
+        a.a12 = fma(L.K2T, u, fma(-(dx * dy), Tv, a.a12));
+    }
+}
+
 // ---- SIS: alpha = b0 (dx,dy)/R, H = b0/R^3 [[dy^2,-dx dy],[-dx dy,dx^2]]; zero at R = 0 ---
 template <bool GRAD, bool HESS>
 __device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc &a) {
@@ -125,8 +181,10 @@ __device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc
     }
 }
 
-template <bool GRAD, bool HESS>
-__global__ void __launch_bounds__(THREADS) superpose_kernel(const EvalParams P) {
+// EXTREME: the model list holds CLS_EXTREME lenses (launch_eval looks at the class ranges); the
+// common instantiations carry none of that code or its registers.
+template <bool GRAD, bool HESS, bool EXTREME>
+__global__ void __launch_bounds__(THREADS, EXTREME ? 1 : LH_MINB) superpose_kernel(const EvalParams P) {
     __shared__ LensK tile[TL];
     __shared__ SmemTables tb;
 
@@ -168,6 +226,7 @@ __global__ void __launch_bounds__(THREADS) superpose_kernel(const EvalParams P) 
             // class sub-ranges inside this tile (type-pure loops, no per-lens branch)
             const int e0 = min(max(rg.begin[1] - base, 0), n);  // end of dPIE
             const int e1 = min(max(rg.begin[2] - base, 0), n);  // end of NSIE
+            const int e2 = min(max(rg.begin[3] - base, 0), n);  // end of SIS
             for (int l = 0; l < e0; ++l) {
 #pragma unroll
                 for (int k = 0; k < PX; ++k) dpie_term<GRAD, HESS>(tile[l], X[k], Y, acc[k], tb);
@@ -176,16 +235,21 @@ __global__ void __launch_bounds__(THREADS) superpose_kernel(const EvalParams P) 
 #pragma unroll
                 for (int k = 0; k < PX; ++k) nsie_term<GRAD, HESS>(tile[l], X[k], Y, acc[k], tb);
             }
-            for (int l = e1; l < n; ++l) {
+            for (int l = e1; l < e2; ++l) {
 #pragma unroll
                 for (int k = 0; k < PX; ++k) sis_term<GRAD, HESS>(tile[l], X[k], Y, acc[k]);
+            }
+            if (EXTREME) {
+                for (int l = e2; l < n; ++l) {
+#pragma unroll
+                    for (int k = 0; k < PX; ++k) extreme_term<GRAD, HESS>(tile[l], X[k], Y, acc[k]);
+                }
             }
         }
 
         // a5: epilogue in registers, then stores of the requested planes only
         if (j < P.ny && i0 < P.nx) {
             const size_t idx = (size_t)model * P.plane + (size_t)j * P.nx + i0;
-            const bool two = (i0 + 1 < P.nx);
             double v[9][PX];
 #pragma unroll
             for (int k = 0; k < PX; ++k) {
@@ -207,11 +271,15 @@ __global__ void __launch_bounds__(THREADS) superpose_kernel(const EvalParams P) 
                 if ((pl < 2 && !GRAD) || (pl >= 2 && !HESS)) continue;
                 double *o = P.out[pl];
                 if (o == nullptr) continue;
-                if (two && (reinterpret_cast<uintptr_t>(o + idx) & 15u) == 0) {  // 16-byte aligned double2
-                    *reinterpret_cast<double2 *>(o + idx) = make_double2(v[pl][0], v[pl][1]);
-                } else {
-                    o[idx] = v[pl][0];
-                    if (two) o[idx + 1] = v[pl][1];
+                const bool al = (reinterpret_cast<uintptr_t>(o + idx) & 15u) == 0;  // 16-byte aligned double2
+#pragma unroll
+                for (int k = 0; k < PX; k += 2) {
+                    if (al && i0 + k + 1 < P.nx) {
+                        *reinterpret_cast<double2 *>(o + idx + k) = make_double2(v[pl][k], v[pl][k + 1]);
+                    } else {
+                        if (i0 + k < P.nx) o[idx + k] = v[pl][k];
+                        if (i0 + k + 1 < P.nx) o[idx + k + 1] = v[pl][k + 1];
+                    }
                 }
             }
         }
@@ -228,12 +296,21 @@ cudaError_t launch_eval(const EvalParams &P_in, cudaStream_t stream) {
     const bool grad = P.out[0] || P.out[1];
     bool hess = false;
     for (int k = 2; k < 9; ++k) hess = hess || P.out[k];
-    if (grad && hess)
-        superpose_kernel<true, true><<<grid, block, 0, stream>>>(P);
-    else if (grad)
-        superpose_kernel<true, false><<<grid, block, 0, stream>>>(P);
-    else
-        superpose_kernel<false, true><<<grid, block, 0, stream>>>(P);
+    if (P.any_extreme) {
+        if (grad && hess)
+            superpose_kernel<true, true, true><<<grid, block, 0, stream>>>(P);
+        else if (grad)
+            superpose_kernel<true, false, true><<<grid, block, 0, stream>>>(P);
+        else
+            superpose_kernel<false, true, true><<<grid, block, 0, stream>>>(P);
+    } else {
+        if (grad && hess)
+            superpose_kernel<true, true, false><<<grid, block, 0, stream>>>(P);
+        else if (grad)
+            superpose_kernel<true, false, false><<<grid, block, 0, stream>>>(P);
+        else
+            superpose_kernel<false, true, false><<<grid, block, 0, stream>>>(P);
+    }
     return cudaGetLastError();
 }
 

@@ -12,6 +12,7 @@ struct EvalParams {
     const ModelRanges *ranges;  // [nmodel]
     const MathTables *math;     // device copy of the atan / atanh reduction tables
     int nlens, nmodel;
+    int any_extreme;            // some model holds CLS_EXTREME lenses (selects the kernel instantiation)
     double x0, y0, dx;
     int nx, ny;
     long long plane;  // nx*ny

@@ -100,11 +100,24 @@ LH_HD void rsqrt_sqrt(double v, double &w, double &iw) {
     w = v * iw;
 }
 
-// atan(n/d) for d > 0 and any finite n.                                12 FP64 + 2 MUFU
+// |x| and copysign as integer operations on the high word (ALU pipe, not the FP64 pipe)
+LH_HD double fabs_i(double x) { return mk64(hi32(x) & 0x7fffffff, lo32(x)); }
+LH_HD double copysign_i(double mag, double sgn) {
+    return mk64((hi32(mag) & 0x7fffffff) | (hi32(sgn) & (int)0x80000000), lo32(mag));
+}
+// a > b for two non-negative doubles: their bit patterns order like 64-bit integers
+LH_HD bool gt_nonneg(double a, double b) {
+#ifdef __CUDA_ARCH__
+    return __double_as_longlong(a) > __double_as_longlong(b);
+#else
+    int64_t x, y; std::memcpy(&x, &a, 8); std::memcpy(&y, &b, 8); return x > y;
+#endif
+}
+
+// atan(n/d) for d > 0 and any finite n.  Branch-free.                  12 FP64 + 2 MUFU
 LH_HD double atan_nd(double n, double d, const double2 *__restrict__ tab) {
-    const double an = fabs(n);
-    // |n| > d as an integer comparison of two non-negative doubles (ALU pipe, not FP64)
-    const bool swap = (hi32(an) > hi32(d)) || (hi32(an) == hi32(d) && (uint32_t)lo32(an) > (uint32_t)lo32(d));
+    const double an = fabs_i(n);
+    const bool swap = gt_nonneg(an, d);
     const double hi = swap ? an : d, lo = swap ? d : an;  // t = lo/hi in [0, 1]
     // index: round(128 t) from the seed quotient, read from the low word after adding 1.5 * 2^45
     const double kk = fma(lo, rcp_seed(hi), 52776558133248.0);
@@ -114,28 +127,30 @@ LH_HD double atan_nd(double n, double d, const double2 *__restrict__ tab) {
     const double z = num * rcp(den);  // |z| <= 2^-8
     const double z2 = z * z;
     const double p = fma(z2, fma(z2, 0.2, -1.0 / 3.0), 1.0);
+    // swap: atan(t) = pi/2 - atan(1/t)  ->  res = base -+ (atan c + z p), one FMA either way
+    const double sg = swap ? -1.0 : 1.0, base = swap ? 1.5707963267948966 : 0.0;
     const double r = fma(z, p, ca.y);
-    const double res = swap ? (1.5707963267948966 - r) : r;
-    return copysign(res, n);
+    return copysign_i(fma(sg, r, base), n);
 }
 
-// atanh(n/d) for |n| < d.                                             12 FP64 + 2 MUFU
+// atanh(n/d) for |n| < d with (d+|n|)/(d-|n|) < 2^16.  Branch-free.   13 FP64 + 2 MUFU
 // The bin is chosen in the ratio domain q = (d+|n|)/(d-|n|) (so that the exponent of q does the
 // coarse part of the logarithm), the reduction is done in the u = n/d domain against
 // c' = (c-1)/(c+1), atanh(c') = 1/2 ln(c): both FMAs below see the exact n and d.
+// The host packer (lh_pack.cpp) routes every lens whose ellipticity could push q past the table
+// into the CLS_EXTREME class, which does not come through here; the index is clamped all the same.
 LH_HD double atanh_nd(double n, double d, const double2 *__restrict__ tab) {
-    const double an = fabs(n);                          // odd symmetry: q >= 1
+    const double an = fabs_i(n);                        // odd symmetry: q >= 1
     const double a = d + an, b = d - an;
     const double q0 = a * rcp_seed(b);                  // q to 1e-6
-    const int hr = (hi32(q0) + 0x2000) & 0xffffc000;    // q rounded to 6 mantissa bits = c
-    const unsigned j = (unsigned)((hr >> 14) - (1023 << 6));
-    if (j >= (unsigned)LN_N) return copysign(0.5 * log(a / b), n);  // q >= 2^16 (e-hat -> 1 only), inf, nan
+    const int hr = hi32(q0) + 0x2000;                   // q rounded to 6 mantissa bits = c
+    const int j = max(0, min((hr >> 14) - (1023 << 6), LN_N - 1));
     const double2 ca = tab[j];                          // {c', atanh c'}
     const double num = fma(-ca.x, d, an), den = fma(-ca.x, an, d);
     const double s = num * rcp(den);                    // |s| <= 2^-8
     const double s2 = s * s;
     const double p = fma(s2, fma(s2, 0.2, 1.0 / 3.0), 1.0);
-    return copysign(fma(s, p, ca.y), n);
+    return copysign_i(fma(s, p, ca.y), n);
 }
 
 // host: fill the tables (libm, correctly rounded enough: they are constants of the library)

@@ -36,6 +36,8 @@ static int classify(const lh_lens &L, int idx, int model, char *err, int errlen)
     if (!(L.ellipticity >= 0.0 && L.ellipticity < 1.0)) return fail("ellipticity outside [0,1)");
     if (!(L.rcore > 0.0)) return fail("rcore must be > 0");
     if (L.type == LH_DPIE && !(L.rcut > L.rcore)) return fail("dPIE needs rcut > rcore");
+    const double e = L.ellipticity;
+    if (e / (1.0 + std::sqrt(1.0 - e * e)) > EXTREME_EPS) return CLS_EXTREME;
     return L.type == LH_DPIE ? CLS_DPIE : CLS_NSIE;
 }
 
@@ -52,7 +54,7 @@ static void fill(const lh_lens &L, int cls, LensK &K) {
     const double eps = e / (1.0 + std::sqrt(1.0 - e * e));  // reading 8c-2
     const double o = 1.0 - eps * eps, p = (1.0 + eps) * (1.0 + eps), m = (1.0 - eps) * (1.0 - eps);
     const double rc = L.rcore;
-    const bool cut = (cls == CLS_DPIE);
+    const bool cut = (L.type == LH_DPIE);
     const double rt = cut ? L.rcut : 0.0;
     const double T = cut ? L.b0 * rt / (rt - rc) : L.b0;
     const double c2 = std::cos(2.0 * L.theta), s2 = std::sin(2.0 * L.theta);
@@ -75,6 +77,7 @@ static void fill(const lh_lens &L, int cls, LensK &K) {
     K.cG = K.c * G;
     K.sG = K.s * G;
     K.T = T;
+    K.eps = eps;
     K.orc2 = 2.0 * o * rc;
     K.ort2 = 2.0 * o * rt;
     K.c0c = 2.0 * (1.0 + eps * eps) * rc * rc;
@@ -85,7 +88,7 @@ static void fill(const lh_lens &L, int cls, LensK &K) {
 
 int pack_model(const void *records, int n, LensK *out, ModelRanges *ranges, char *err, int errlen, int model) {
     const lh_lens *L = static_cast<const lh_lens *>(records);
-    int count[CLS_COUNT] = {0, 0, 0};
+    int count[CLS_COUNT] = {0, 0, 0, 0};
     // pass 1: validate + count (stable counting sort keeps index order inside a class)
     for (int i = 0; i < n; ++i) {
         int cls = classify(L[i], i, model, err, errlen);

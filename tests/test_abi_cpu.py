@@ -48,11 +48,27 @@ def test_struct_layouts_match_header():
 def test_pack_sorts_by_class_and_is_stable():
     c = li.config(2)
     table, begin = lh.lh_pack_model(c.lenses)
-    assert list(begin) == [0, 402, 451, 500]
+    assert list(begin) == [0, 402, 451, 500, 500]  # dPIE | NSIE | SIS | extreme-ellipticity
     for cls, t in ((0, li.DPIE), (1, li.NSIE), (2, li.SIS)):
         src = c.lenses[c.lenses["type"] == t]
         sl = table[begin[cls]:begin[cls + 1]]
         assert np.array_equal(sl[:, 0], src["x"]) and np.array_equal(sl[:, 1], src["y"])  # index order kept
+
+
+def test_pack_routes_extreme_ellipticity_to_its_own_class():
+    """eps > 0.96 (e-hat > 0.99917, axis ratio < 0.0204) leaves the fast dPIE / NSIE classes (lh_pack.h)."""
+    L = li.make_lenses(5)
+    L[0] = (li.DPIE, 0, 0.0, 0.0, 0.9991, 0.1, 0.1, 10.0, 1.0)   # eps = 0.9585: fast
+    L[1] = (li.DPIE, 0, 1.0, 0.0, 0.9993, 0.1, 0.1, 10.0, 1.0)   # eps = 0.9633: extreme
+    L[2] = (li.NSIE, 0, 2.0, 0.0, 0.99999, 0.1, 0.1, 0.0, 1.0)   # extreme, no cut
+    L[3] = (li.SIS, 0, 3.0, 0.0, 0.99999, 0.0, 0.0, 0.0, 1.0)    # SIS ignores ellipticity
+    L[4] = (li.NSIE, 0, 4.0, 0.0, 0.5, 0.1, 0.1, 0.0, 1.0)
+    t, begin = lh.lh_pack_model(L)
+    assert list(begin) == [0, 1, 2, 3, 5]
+    assert list(t[:, 0]) == [0.0, 4.0, 3.0, 1.0, 2.0]
+    assert t[3, 7] == 100.0 and t[4, 7] == 0.0  # rt^2; 0 marks "no cut term" in the extreme class
+    e = 0.9993
+    assert t[3, 17] == e / (1 + math.sqrt(1 - e * e))  # eps slot
 
 
 def test_pack_constants():
