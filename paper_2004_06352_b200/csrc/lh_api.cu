@@ -8,30 +8,33 @@
 #include <cstring>
 #include <mutex>
 #include <new>
+#include <vector>
 
 #include "../../include/lh.h"
 #include "lh_kernels.h"
 
 namespace {
 
-using lh::EvalParams;
 using lh::LensK;
 using lh::ModelRanges;
 
-// Per-host-thread state: stream, last error, and the staging buffers for the packed
-// table.  The pinned staging area may only be rewritten once the previous H2D copy has
-// finished (ev_copied); the device table may only be overwritten once the previous
-// kernel has finished reading it, which stream order guarantees on one stream and
-// ev_done + cudaStreamWaitEvent guarantees across a stream change.
+// Per-host-thread state: stream, last error, the host buffer the lens tables are packed
+// into, and two cached device buffers.  The packed records travel to the device inside the
+// kernel parameters (lh_kernels.h), copied by the launch itself, so the host buffer may be
+// rewritten as soon as launch_eval returns.  `d_carry` (accumulators handed from one lens
+// chunk of a model to the next) is reused across calls: stream order protects it on one
+// stream, ev_done + cudaStreamWaitEvent across a stream change.
 struct Context {
     cudaStream_t stream = nullptr;
     char err[512] = {0};
     long long launches = 0;
 
-    void *h_stage = nullptr;  // pinned: [ranges | table]
-    void *d_stage = nullptr;
-    size_t stage_bytes = 0;
-    cudaEvent_t ev_copied = nullptr, ev_done = nullptr;
+    std::vector<LensK> h_table;
+    std::vector<ModelRanges> h_ranges;
+
+    double *d_carry = nullptr;
+    size_t carry_bytes = 0;
+    cudaEvent_t ev_done = nullptr;
     cudaStream_t last_stream = nullptr;
     bool busy = false;
 
@@ -111,66 +114,54 @@ int check_device_ptr(const double *p, const char *name) {
 
 const char *PLANE_NAMES[NPLANES] = {"ax", "ay", "a11", "a12", "a22", "kappa", "gamma1", "gamma2", "mu"};
 
-// Validate + pack + stage + launch.  `dev_out` are device planes (already checked).
+// Validate + pack + launch.  `dev_out` are device planes (already checked).
 int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *dev_out[NPLANES]) {
-    const size_t n_total = (size_t)nmodel * (size_t)nlens;
-    const size_t ranges_bytes = ((size_t)nmodel * sizeof(ModelRanges) + 15) & ~size_t(15);
-    const size_t need = ranges_bytes + n_total * sizeof(LensK);
-
-    if (!ctx.ev_copied) {
-        CU(cudaEventCreateWithFlags(&ctx.ev_copied, cudaEventDisableTiming));
-        CU(cudaEventCreateWithFlags(&ctx.ev_done, cudaEventDisableTiming));
+    // a1: pack on the host (validates; nothing is enqueued if any lens is rejected)
+    try {
+        ctx.h_table.resize((size_t)nmodel * (size_t)nlens);
+        ctx.h_ranges.resize((size_t)nmodel);
+    } catch (const std::bad_alloc &) {
+        return fail(LH_EINVAL, "out of host memory packing %d x %d lenses", nmodel, nlens);
     }
-    if (ctx.busy) CU(cudaEventSynchronize(ctx.ev_copied));  // staging area free again
-    if (need > ctx.stage_bytes) {
-        if (ctx.busy) CU(cudaEventSynchronize(ctx.ev_done));  // old device table no longer read
-        if (ctx.h_stage) cudaFreeHost(ctx.h_stage);
-        if (ctx.d_stage) cudaFree(ctx.d_stage);
-        ctx.h_stage = ctx.d_stage = nullptr;
-        ctx.stage_bytes = 0;
-        const size_t cap = need + need / 2 + 4096;
-        CU(cudaMallocHost(&ctx.h_stage, cap));
-        CU(cudaMalloc(&ctx.d_stage, cap));
-        ctx.stage_bytes = cap;
-    }
-
-    // a1: pack on the host straight into the pinned staging area
-    ModelRanges *h_ranges = static_cast<ModelRanges *>(ctx.h_stage);
-    LensK *h_table = reinterpret_cast<LensK *>(static_cast<char *>(ctx.h_stage) + ranges_bytes);
-    bool any_extreme = false;
     for (int m = 0; m < nmodel; ++m) {
-        if (lh::pack_model(lenses + (size_t)m * nlens, nlens, h_table + (size_t)m * nlens, h_ranges + m, ctx.err,
-                           sizeof(ctx.err), m) != 0)
-            return LH_EINVAL;  // message already written; nothing enqueued
-        any_extreme |= h_ranges[m].begin[lh::CLS_EXTREME + 1] > h_ranges[m].begin[lh::CLS_EXTREME];
+        if (lh::pack_model(lenses + (size_t)m * nlens, nlens, ctx.h_table.data() + (size_t)m * nlens,
+                           ctx.h_ranges.data() + m, ctx.err, sizeof(ctx.err), m) != 0)
+            return LH_EINVAL;  // message already written
     }
 
     cudaStream_t s = ctx.stream;
-    if (ctx.busy && ctx.last_stream != s) CU(cudaStreamWaitEvent(s, ctx.ev_done, 0));
-    CU(cudaMemcpyAsync(ctx.d_stage, ctx.h_stage, need, cudaMemcpyHostToDevice, s));
-    CU(cudaEventRecord(ctx.ev_copied, s));
+    if (!ctx.ev_done) CU(cudaEventCreateWithFlags(&ctx.ev_done, cudaEventDisableTiming));
+    const size_t carry_need = nlens > lh::LAUNCH_RECORDS ? (size_t)5 * g->nx * g->ny * sizeof(double) : 0;
+    if (carry_need > ctx.carry_bytes) {
+        if (ctx.busy) CU(cudaEventSynchronize(ctx.ev_done));  // the old buffer is no longer in use
+        if (ctx.d_carry) cudaFree(ctx.d_carry);
+        ctx.d_carry = nullptr;
+        ctx.carry_bytes = 0;
+        CU(cudaMalloc(&ctx.d_carry, carry_need));
+        ctx.carry_bytes = carry_need;
+    }
+    if (carry_need && ctx.busy && ctx.last_stream != s) CU(cudaStreamWaitEvent(s, ctx.ev_done, 0));
 
     int dev = 0;
     CU(cudaGetDevice(&dev));
     cudaError_t terr;
-    EvalParams P;
-    P.math = device_math_tables(dev, &terr);
-    if (!P.math) return fail(LH_ECUDA, "math tables: %s", cudaGetErrorString(terr));
-    P.ranges = static_cast<const ModelRanges *>(ctx.d_stage);
-    P.table = reinterpret_cast<const LensK *>(static_cast<char *>(ctx.d_stage) + ranges_bytes);
-    P.nlens = nlens;
-    P.nmodel = nmodel;
-    P.any_extreme = any_extreme ? 1 : 0;
-    P.x0 = g->x0; P.y0 = g->y0; P.dx = g->dx;
-    P.nx = g->nx; P.ny = g->ny;
-    P.plane = (long long)g->nx * g->ny;
-    for (int k = 0; k < NPLANES; ++k) P.out[k] = dev_out[k];
-    P.tiles_x = P.tiles_y = 0;
-    CU(lh::launch_eval(P, s));
-    ++ctx.launches;
-    CU(cudaEventRecord(ctx.ev_done, s));
-    ctx.busy = true;
-    ctx.last_stream = s;
+    lh::EvalJob J;
+    J.math = device_math_tables(dev, &terr);
+    if (!J.math) return fail(LH_ECUDA, "math tables: %s", cudaGetErrorString(terr));
+    J.table = ctx.h_table.data();
+    J.ranges = ctx.h_ranges.data();
+    J.nlens = nlens;
+    J.nmodel = nmodel;
+    J.x0 = g->x0; J.y0 = g->y0; J.dx = g->dx;
+    J.nx = g->nx; J.ny = g->ny;
+    for (int k = 0; k < NPLANES; ++k) J.out[k] = dev_out[k];
+    J.carry = ctx.d_carry;
+    CU(lh::launch_eval(J, s, &ctx.launches));
+    if (carry_need) {
+        CU(cudaEventRecord(ctx.ev_done, s));
+        ctx.busy = true;
+        ctx.last_stream = s;
+    }
     return LH_OK;
 }
 

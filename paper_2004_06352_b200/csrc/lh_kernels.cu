@@ -19,6 +19,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <cstring>
 
 #include "lh_kernels.h"
 
@@ -37,7 +38,6 @@ constexpr int PX = LH_PX;
 constexpr int TILE_W = 32 * PX;    // one warp spans 32*PX pixels of a row
 constexpr int TILE_H = LH_WARPS;
 constexpr int THREADS = 32 * TILE_H;
-constexpr int TL = 64;             // lenses per shared-memory tile
 static_assert(PX % 2 == 0, "PX must be even (double2 stores)");
 
 struct Acc {
@@ -181,11 +181,18 @@ __device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc
     }
 }
 
-// EXTREME: the model list holds CLS_EXTREME lenses (launch_eval looks at the class ranges); the
+// EXTREME: the launch holds CLS_EXTREME lenses (launch_eval looks at the class ranges); the
 // common instantiations carry none of that code or its registers.
+//
+// The lens records of a launch arrive BY VALUE in the kernel parameters (constant bank 0):
+// the lens index is warp-uniform, so every record field is fetched by the uniform datapath
+// (LDCU) into a uniform register and enters the FP64 instructions as their one uniform
+// operand.  That matters because the B200 FP64 pipe issues a warp instruction every 2 cycles
+// only while it reads at most two distinct vector registers; an FMA with three costs 3
+// (profiles/r01_fp64_operand_probe.md).  A record staged in shared memory would land in
+// vector registers and make almost every FMA of the lens algebra a 3-register one.
 template <bool GRAD, bool HESS, bool EXTREME>
-__global__ void __launch_bounds__(THREADS, EXTREME ? 1 : LH_MINB) superpose_kernel(const EvalParams P) {
-    __shared__ LensK tile[TL];
+__global__ void __launch_bounds__(THREADS, EXTREME ? 1 : LH_MINB) superpose_kernel(const __grid_constant__ LaunchParams P) {
     __shared__ SmemTables tb;
 
     // reduction tables of atan / atanh: global (L2-resident, 18 KB) -> shared, once per CTA
@@ -199,6 +206,7 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : LH_MINB) superpose_kern
     const int tx = blockIdx.x % P.tiles_x, ty = blockIdx.x / P.tiles_x;
     const int i0 = tx * TILE_W + lane * PX;
     const int j = ty * TILE_H + warp;
+    const bool inside = j < P.ny && i0 < P.nx;
 
     // a2: pixel coordinates from the grid definition (no coordinate array in memory)
     double X[PX];
@@ -206,112 +214,177 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : LH_MINB) superpose_kern
     for (int k = 0; k < PX; ++k) X[k] = fma((double)(i0 + k), P.dx, P.x0);
     const double Y = fma((double)j, P.dx, P.y0);
 
-    for (int model = blockIdx.y; model < P.nmodel; model += gridDim.y) {
-        const LensK *table = P.table + (size_t)model * P.nlens;
-        const ModelRanges rg = P.ranges[model];
+    const int m = blockIdx.y;  // model inside this launch
+    const size_t pix = (size_t)j * P.nx + i0;
 
-        Acc acc[PX];
+    // accumulators: zero on the first lens chunk of a model, else carried over from the previous launch
+    Acc acc[PX];
 #pragma unroll
-        for (int k = 0; k < PX; ++k) acc[k] = Acc{0.0, 0.0, 0.0, 0.0, 0.0};
-
-        for (int base = 0; base < P.nlens; base += TL) {
-            const int n = min(TL, P.nlens - base);
-            __syncthreads();  // previous tile fully consumed
-            {
-                const double2 *src = reinterpret_cast<const double2 *>(table + base);
-                double2 *dst = reinterpret_cast<double2 *>(tile);
-                for (int t = threadIdx.x; t < n * (LENSK_DOUBLES / 2); t += THREADS) dst[t] = __ldg(src + t);
-            }
-            __syncthreads();
-            // class sub-ranges inside this tile (type-pure loops, no per-lens branch)
-            const int e0 = min(max(rg.begin[1] - base, 0), n);  // end of dPIE
-            const int e1 = min(max(rg.begin[2] - base, 0), n);  // end of NSIE
-            const int e2 = min(max(rg.begin[3] - base, 0), n);  // end of SIS
-            for (int l = 0; l < e0; ++l) {
+    for (int k = 0; k < PX; ++k) acc[k] = Acc{0.0, 0.0, 0.0, 0.0, 0.0};
+    if (!P.first && inside) {
 #pragma unroll
-                for (int k = 0; k < PX; ++k) dpie_term<GRAD, HESS>(tile[l], X[k], Y, acc[k], tb);
-            }
-            for (int l = e0; l < e1; ++l) {
-#pragma unroll
-                for (int k = 0; k < PX; ++k) nsie_term<GRAD, HESS>(tile[l], X[k], Y, acc[k], tb);
-            }
-            for (int l = e1; l < e2; ++l) {
-#pragma unroll
-                for (int k = 0; k < PX; ++k) sis_term<GRAD, HESS>(tile[l], X[k], Y, acc[k]);
-            }
-            if (EXTREME) {
-                for (int l = e2; l < n; ++l) {
-#pragma unroll
-                    for (int k = 0; k < PX; ++k) extreme_term<GRAD, HESS>(tile[l], X[k], Y, acc[k]);
-                }
+        for (int k = 0; k < PX; ++k) {
+            if (i0 + k < P.nx) {
+                const double *c = P.carry + pix + k;
+                if (GRAD) { acc[k].ax = c[0]; acc[k].ay = c[P.plane]; }
+                if (HESS) { acc[k].S = c[2 * P.plane]; acc[k].Dl = c[3 * P.plane]; acc[k].a12 = c[4 * P.plane]; }
             }
         }
+    }
+    __syncthreads();  // tables staged
 
-        // a5: epilogue in registers, then stores of the requested planes only
-        if (j < P.ny && i0 < P.nx) {
-            const size_t idx = (size_t)model * P.plane + (size_t)j * P.nx + i0;
-            double v[9][PX];
+    // class sub-ranges of this model's records (type-pure loops, no per-lens branch)
+    const int b = m * P.stride;
+    const int e0 = b + P.cls_end[m][0];  // end of dPIE
+    const int e1 = b + P.cls_end[m][1];  // end of NSIE
+    const int e2 = b + P.cls_end[m][2];  // end of SIS
+    for (int l = b; l < e0; ++l) {
 #pragma unroll
-            for (int k = 0; k < PX; ++k) {
-                const double kap = 0.5 * acc[k].S, g1 = 0.5 * acc[k].Dl, g2 = acc[k].a12;
-                const double omk = 1.0 - kap;
-                const double det = fma(omk, omk, -fma(g1, g1, g2 * g2));
-                v[0][k] = acc[k].ax;
-                v[1][k] = acc[k].ay;
-                v[2][k] = kap + g1;  // a11
-                v[3][k] = g2;        // a12
-                v[4][k] = kap - g1;  // a22
-                v[5][k] = kap;
-                v[6][k] = g1;
-                v[7][k] = g2;
-                v[8][k] = 1.0 / det;
+        for (int k = 0; k < PX; ++k) dpie_term<GRAD, HESS>(P.table[l], X[k], Y, acc[k], tb);
+    }
+    for (int l = e0; l < e1; ++l) {
+#pragma unroll
+        for (int k = 0; k < PX; ++k) nsie_term<GRAD, HESS>(P.table[l], X[k], Y, acc[k], tb);
+    }
+    for (int l = e1; l < e2; ++l) {
+#pragma unroll
+        for (int k = 0; k < PX; ++k) sis_term<GRAD, HESS>(P.table[l], X[k], Y, acc[k]);
+    }
+    if (EXTREME) {
+        const int e3 = b + P.cls_end[m][3];
+        for (int l = e2; l < e3; ++l) {
+#pragma unroll
+            for (int k = 0; k < PX; ++k) extreme_term<GRAD, HESS>(P.table[l], X[k], Y, acc[k]);
+        }
+    }
+    if (!inside) return;
+
+    if (!P.last) {  // more lens chunks of this model follow: park the accumulators
+#pragma unroll
+        for (int k = 0; k < PX; ++k) {
+            if (i0 + k < P.nx) {
+                double *c = P.carry + pix + k;
+                if (GRAD) { c[0] = acc[k].ax; c[P.plane] = acc[k].ay; }
+                if (HESS) { c[2 * P.plane] = acc[k].S; c[3 * P.plane] = acc[k].Dl; c[4 * P.plane] = acc[k].a12; }
             }
+        }
+        return;
+    }
+
+    // a5: epilogue in registers, then stores of the requested planes only
+    const size_t idx = (size_t)(P.model0 + m) * P.plane + pix;
+    double v[9][PX];
 #pragma unroll
-            for (int pl = 0; pl < 9; ++pl) {
-                if ((pl < 2 && !GRAD) || (pl >= 2 && !HESS)) continue;
-                double *o = P.out[pl];
-                if (o == nullptr) continue;
-                const bool al = (reinterpret_cast<uintptr_t>(o + idx) & 15u) == 0;  // 16-byte aligned double2
+    for (int k = 0; k < PX; ++k) {
+        const double kap = 0.5 * acc[k].S, g1 = 0.5 * acc[k].Dl, g2 = acc[k].a12;
+        const double omk = 1.0 - kap;
+        const double det = fma(omk, omk, -fma(g1, g1, g2 * g2));
+        v[0][k] = acc[k].ax;
+        v[1][k] = acc[k].ay;
+        v[2][k] = kap + g1;  // a11
+        v[3][k] = g2;        // a12
+        v[4][k] = kap - g1;  // a22
+        v[5][k] = kap;
+        v[6][k] = g1;
+        v[7][k] = g2;
+        v[8][k] = 1.0 / det;
+    }
 #pragma unroll
-                for (int k = 0; k < PX; k += 2) {
-                    if (al && i0 + k + 1 < P.nx) {
-                        *reinterpret_cast<double2 *>(o + idx + k) = make_double2(v[pl][k], v[pl][k + 1]);
-                    } else {
-                        if (i0 + k < P.nx) o[idx + k] = v[pl][k];
-                        if (i0 + k + 1 < P.nx) o[idx + k + 1] = v[pl][k + 1];
-                    }
-                }
+    for (int pl = 0; pl < 9; ++pl) {
+        if ((pl < 2 && !GRAD) || (pl >= 2 && !HESS)) continue;
+        double *o = P.out[pl];
+        if (o == nullptr) continue;
+        const bool al = (reinterpret_cast<uintptr_t>(o + idx) & 15u) == 0;  // 16-byte aligned double2
+#pragma unroll
+        for (int k = 0; k < PX; k += 2) {
+            if (al && i0 + k + 1 < P.nx) {
+                *reinterpret_cast<double2 *>(o + idx + k) = make_double2(v[pl][k], v[pl][k + 1]);
+            } else {
+                if (i0 + k < P.nx) o[idx + k] = v[pl][k];
+                if (i0 + k + 1 < P.nx) o[idx + k + 1] = v[pl][k + 1];
             }
         }
     }
 }
 
-cudaError_t launch_eval(const EvalParams &P_in, cudaStream_t stream) {
-    EvalParams P = P_in;
-    P.tiles_x = (P.nx + TILE_W - 1) / TILE_W;
-    P.tiles_y = (P.ny + TILE_H - 1) / TILE_H;
-    const long long tiles = (long long)P.tiles_x * P.tiles_y;
-    if (tiles > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    dim3 grid((unsigned)tiles, (unsigned)min(P.nmodel, 65535), 1), block(THREADS, 1, 1);
-    const bool grad = P.out[0] || P.out[1];
-    bool hess = false;
-    for (int k = 2; k < 9; ++k) hess = hess || P.out[k];
-    if (P.any_extreme) {
-        if (grad && hess)
-            superpose_kernel<true, true, true><<<grid, block, 0, stream>>>(P);
-        else if (grad)
-            superpose_kernel<true, false, true><<<grid, block, 0, stream>>>(P);
-        else
-            superpose_kernel<false, true, true><<<grid, block, 0, stream>>>(P);
-    } else {
-        if (grad && hess)
-            superpose_kernel<true, true, false><<<grid, block, 0, stream>>>(P);
-        else if (grad)
-            superpose_kernel<true, false, false><<<grid, block, 0, stream>>>(P);
-        else
-            superpose_kernel<false, true, false><<<grid, block, 0, stream>>>(P);
-    }
+template <bool GRAD, bool HESS, bool EXTREME>
+static cudaError_t launch_one(const LaunchParams &P, dim3 grid, cudaStream_t stream) {
+    superpose_kernel<GRAD, HESS, EXTREME><<<grid, dim3(THREADS, 1, 1), 0, stream>>>(P);
     return cudaGetLastError();
+}
+
+// Host side of a6 and of the lens chunking: cut the packed tables into launches of at most
+// LAUNCH_RECORDS records.  Models with few lenses share a launch (blockIdx.y = model); a model
+// with more lenses than fit is evaluated by consecutive launches that hand the accumulators on
+// through `carry` (stream order makes that safe).
+cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launches) {
+    thread_local LaunchParams Q;  // 32 KB: kept off the stack
+    Q.x0 = J.x0; Q.y0 = J.y0; Q.dx = J.dx;
+    Q.nx = J.nx; Q.ny = J.ny;
+    Q.plane = (long long)J.nx * J.ny;
+    for (int k = 0; k < 9; ++k) Q.out[k] = J.out[k];
+    Q.carry = J.carry;
+    Q.math = J.math;
+    Q.tiles_x = (J.nx + TILE_W - 1) / TILE_W;
+    const long long tiles = (long long)Q.tiles_x * ((J.ny + TILE_H - 1) / TILE_H);
+    if (tiles > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    const bool grad = J.out[0] || J.out[1];
+    bool hess = false;
+    for (int k = 2; k < 9; ++k) hess = hess || J.out[k];
+
+    auto go = [&](int nm, bool extreme) -> cudaError_t {
+        dim3 grid((unsigned)tiles, (unsigned)nm, 1);
+        ++*launches;
+        if (extreme) {
+            if (grad && hess) return launch_one<true, true, true>(Q, grid, stream);
+            if (grad) return launch_one<true, false, true>(Q, grid, stream);
+            return launch_one<false, true, true>(Q, grid, stream);
+        }
+        if (grad && hess) return launch_one<true, true, false>(Q, grid, stream);
+        if (grad) return launch_one<true, false, false>(Q, grid, stream);
+        return launch_one<false, true, false>(Q, grid, stream);
+    };
+
+    const int n = J.nlens;
+    if (n <= LAUNCH_RECORDS) {
+        // whole models per launch
+        const int per = n > 0 ? LAUNCH_RECORDS / n : LAUNCH_MODELS;
+        const int mpl = per < LAUNCH_MODELS ? per : LAUNCH_MODELS;
+        for (int m0 = 0; m0 < J.nmodel; m0 += mpl) {
+            const int nm = (J.nmodel - m0 < mpl) ? J.nmodel - m0 : mpl;
+            bool extreme = false;
+            for (int m = 0; m < nm; ++m) {
+                const ModelRanges &rg = J.ranges[m0 + m];
+                for (int c = 0; c < CLS_COUNT; ++c) Q.cls_end[m][c] = (unsigned short)rg.begin[c + 1];
+                extreme = extreme || rg.begin[CLS_EXTREME + 1] > rg.begin[CLS_EXTREME];
+            }
+            if (n > 0) std::memcpy(Q.table, J.table + (size_t)m0 * n, (size_t)nm * n * sizeof(LensK));
+            Q.model0 = m0; Q.stride = n; Q.first = 1; Q.last = 1;
+            cudaError_t e = go(nm, extreme);
+            if (e != cudaSuccess) return e;
+        }
+        return cudaSuccess;
+    }
+    // one model at a time, balanced lens chunks
+    const int nch = (n + LAUNCH_RECORDS - 1) / LAUNCH_RECORDS;
+    for (int m = 0; m < J.nmodel; ++m) {
+        const ModelRanges &rg = J.ranges[m];
+        for (int c = 0; c < nch; ++c) {
+            const int lo = (int)((long long)n * c / nch), hi = (int)((long long)n * (c + 1) / nch);
+            bool extreme = false;
+            for (int k = 0; k < CLS_COUNT; ++k) {
+                int e = rg.begin[k + 1] - lo;
+                e = e < 0 ? 0 : (e > hi - lo ? hi - lo : e);
+                Q.cls_end[0][k] = (unsigned short)e;
+            }
+            extreme = Q.cls_end[0][CLS_EXTREME] > Q.cls_end[0][CLS_SIS];
+            std::memcpy(Q.table, J.table + (size_t)m * n + lo, (size_t)(hi - lo) * sizeof(LensK));
+            Q.model0 = m; Q.stride = hi - lo; Q.first = (c == 0); Q.last = (c == nch - 1);
+            cudaError_t e = go(1, extreme);
+            if (e != cudaSuccess) return e;
+        }
+    }
+    return cudaSuccess;
 }
 
 // ---- FP64 roofline probe: independent DFMA chains, all SMs, full occupancy -------------------

@@ -7,20 +7,41 @@
 
 namespace lh {
 
-struct EvalParams {
-    const LensK *table;         // [nmodel][nlens], each model sorted by class
-    const ModelRanges *ranges;  // [nmodel]
-    const MathTables *math;     // device copy of the atan / atanh reduction tables
+// Records one launch carries in its kernel parameters (constant bank 0, 32 764 bytes at most):
+// 160 x 192 B of lens constants + 160 x 8 B of class boundaries + a 152-byte header.
+constexpr int LAUNCH_RECORDS = 160;
+constexpr int LAUNCH_MODELS = 160;  // models that may share one launch (blockIdx.y)
+
+struct LaunchParams {
+    double x0, y0, dx;
+    long long plane;         // nx*ny
+    double *out[9];          // ax ay a11 a12 a22 kappa gamma1 gamma2 mu; nullptr = not wanted; [nmodel][ny][nx]
+    double *carry;           // [5][ny][nx] accumulators handed from one lens chunk of a model to the next
+    const MathTables *math;  // device copy of the atan / atanh reduction tables
+    int nx, ny, tiles_x;
+    int model0;              // global index of the launch's first model (blockIdx.y = model - model0)
+    int stride;              // records per model in table[]
+    int first, last;         // this launch holds the first / last lens chunk of its model(s)
+    int pad_;
+    unsigned short cls_end[LAUNCH_MODELS][CLS_COUNT];  // per model: end of each class, relative to its slice
+    LensK table[LAUNCH_RECORDS];
+};
+static_assert(sizeof(LaunchParams) <= 32764, "kernel parameter space");
+
+// One call of the C ABI: nmodel packed tables (host memory) on one grid.
+struct EvalJob {
+    const LensK *table;         // HOST [nmodel][nlens], each model sorted by class
+    const ModelRanges *ranges;  // HOST [nmodel]
+    const MathTables *math;     // DEVICE
     int nlens, nmodel;
-    int any_extreme;            // some model holds CLS_EXTREME lenses (selects the kernel instantiation)
     double x0, y0, dx;
     int nx, ny;
-    long long plane;  // nx*ny
-    double *out[9];   // ax ay a11 a12 a22 kappa gamma1 gamma2 mu; nullptr = not wanted
-    int tiles_x, tiles_y;  // filled by launch_eval
+    double *out[9];  // DEVICE
+    double *carry;   // DEVICE, 5*nx*ny doubles; needed only when nlens > LAUNCH_RECORDS
 };
 
-cudaError_t launch_eval(const EvalParams &P, cudaStream_t stream);
+// Enqueues every launch of the job on `stream`; adds the number of kernels launched to *launches.
+cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launches);
 cudaError_t launch_dfma_probe(int iters, int blocks, double *sink, cudaStream_t stream);
 
 }  // namespace lh
