@@ -146,6 +146,29 @@ int lh_pack_model(const lh_lens *lenses, int n, double *table, int32_t *class_be
  * synchronises).  Used by bench.py as the measured FP64 CUDA-core roofline. */
 int lh_fp64_peak_probe(int iters, double *flops_per_s, double *seconds);
 
+/* HOST evaluation of the kernel's own FP64 primitives (csrc/lh_math.cuh compiles for host and
+ * device; on the host the 20-bit MUFU seeds are emulated by truncated exact quotients), so that
+ * CPU-only tests can pin them against libm / arbitrary precision.  out[k] = fn(a[k], b[k]):
+ *   fn 0  1/a            1  sqrt(a)        2  1/sqrt(a)
+ *      3  atan(a/b), b > 0                 4  atanh(a/b), |a| < b, (b+|a|)/(b-|a|) < 2^16
+ *      5  1/a via the shared-seed pair (a, b)     6  1/a via the shared-seed quadruple (a, b, a+b, 2b)
+ * No CUDA call is made.  LH_EINVAL for an unknown fn or a NULL pointer (b may be NULL for fn 0-2). */
+int lh_math_host_eval(int fn, const double *a, const double *b, size_t n, double *out);
+
+/* Diagnostic behind DESIGN.md sec. 7 (the dispatch-cost model the kernel is written against).
+ * One group = 12 independent warp-wide FP64 instructions (+ `extra` other instructions); every
+ * warp runs `iters` groups with `warps_per_subpartition` (1..16) warps resident per SM
+ * sub-partition on every SM.  *cycles_per_group = elapsed time x max SM clock / (iters x
+ * warps_per_subpartition): 24 means one FP64 instruction per 2 cycles.
+ *   variant 0  FMA with immediate operands      1  FMA, three distinct vector registers
+ *           2  FMA, two distinct registers      3  MUL, two registers
+ *           4  FMA, one uniform operand loaded from the kernel parameters
+ *           5  FMA, one register shared by consecutive instructions
+ *   variant 10/11/12/13  a MUL stream plus `extra` (0, 2, 4, 8) LOP3 / FFMA /
+ *           MUFU.RCP64H+MOV / LDS instructions per group.
+ * Synchronises the set stream.  LH_EINVAL for an unknown variant/extra. */
+int lh_fp64_issue_probe(int variant, int extra, int warps_per_subpartition, int iters, double *cycles_per_group);
+
 /* "lh <major>.<minor> sm_100a" */
 const char *lh_version(void);
 

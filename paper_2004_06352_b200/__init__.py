@@ -8,7 +8,7 @@ missing -- there is no CPU fallback (and it never imports `oracle`).
 Names mirror the C ABI one to one:
     lh_grid_gradient, lh_grid_hessian, lh_lens_maps, lh_grid_gradient_batch,
     lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_pack_model, lh_set_stream,
-    lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_version
+    lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_fp64_issue_probe, lh_math_host_eval, lh_version
 Outputs may be torch CUDA tensors (float64, contiguous), anything with a
 `data_ptr()`, or raw integer device addresses.
 """
@@ -73,6 +73,10 @@ def _load():
         L.lh_last_error.restype = C.c_char_p
         L.lh_launch_count.restype = C.c_longlong
         L.lh_fp64_peak_probe.argtypes = [ci, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.lh_math_host_eval.argtypes = [ci, vp, vp, C.c_size_t, vp]
+        L.lh_math_host_eval.restype = ci
+        L.lh_fp64_issue_probe.argtypes = [ci, ci, ci, ci, C.POINTER(C.c_double)]
+        L.lh_fp64_issue_probe.restype = ci
         L.lh_version.restype = C.c_char_p
         for f in ("lh_grid_gradient", "lh_grid_hessian", "lh_lens_maps", "lh_grid_gradient_batch", "lh_grid_eval",
                   "lh_grid_eval_batch", "lh_grid_eval_host", "lh_set_stream", "lh_fp64_peak_probe"):
@@ -218,6 +222,23 @@ def lh_fp64_peak_probe(iters: int = 4096):
     f, s = C.c_double(), C.c_double()
     _check(_load().lh_fp64_peak_probe(int(iters), C.byref(f), C.byref(s)))
     return f.value, s.value
+
+
+def lh_math_host_eval(fn: int, a, b=None):
+    """HOST evaluation of the kernel's FP64 primitives (include/lh.h); numpy in, numpy out."""
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    bb = None if b is None else np.ascontiguousarray(np.broadcast_to(b, a.shape), dtype=np.float64)
+    out = np.empty_like(a)
+    _check(_load().lh_math_host_eval(int(fn), a.ctypes.data, None if bb is None else bb.ctypes.data, a.size,
+                                     out.ctypes.data))
+    return out
+
+
+def lh_fp64_issue_probe(variant: int, extra: int = 0, warps_per_subpartition: int = 8, iters: int = 20000) -> float:
+    """Dispatch cycles per group of 12 FP64 instructions (+ `extra` others); see include/lh.h."""
+    c = C.c_double()
+    _check(_load().lh_fp64_issue_probe(int(variant), int(extra), int(warps_per_subpartition), int(iters), C.byref(c)))
+    return c.value
 
 
 def lh_version() -> str:

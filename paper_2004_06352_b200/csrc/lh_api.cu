@@ -320,6 +320,59 @@ int lh_fp64_peak_probe(int iters, double *flops_per_s, double *seconds) {
     return LH_OK;
 }
 
+int lh_math_host_eval(int fn, const double *a, const double *b, size_t n, double *out) {
+    ctx.err[0] = 0;
+    if (fn < 0 || fn > 6 || !a || !out || (fn >= 3 && !b)) return fail(LH_EINVAL, "lh_math_host_eval: bad argument");
+    static lh::MathTables tab;
+    static std::once_flag once;
+    std::call_once(once, [] { lh::fill_math_tables(tab); });
+    for (size_t k = 0; k < n; ++k) {
+        double w, iw, i1, i2, i3, i4;
+        switch (fn) {
+            case 0: out[k] = lh::rcp(a[k]); break;
+            case 1: lh::rsqrt_sqrt(a[k], w, iw); out[k] = w; break;
+            case 2: lh::rsqrt_sqrt(a[k], w, iw); out[k] = iw; break;
+            case 3: out[k] = lh::atan_nd(a[k], b[k], tab.at); break;
+            case 4: out[k] = lh::atanh_nd(a[k], b[k], tab.ah); break;
+            case 5: lh::rcp2(a[k], b[k], i1, i2); out[k] = i1; break;
+            default: lh::rcp4(a[k], b[k], a[k] + b[k], 2.0 * b[k], i1, i2, i3, i4); out[k] = i1; break;
+        }
+    }
+    return LH_OK;
+}
+
+int lh_fp64_issue_probe(int variant, int extra, int warps_per_subpartition, int iters, double *cycles_per_group) {
+    ctx.err[0] = 0;
+    if (iters <= 0 || !cycles_per_group || warps_per_subpartition < 1 || warps_per_subpartition > 16)
+        return fail(LH_EINVAL, "lh_fp64_issue_probe: bad argument");
+    int dev = 0, sms = 0, khz = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CU(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev));
+    if (!ctx.d_sink) CU(cudaMalloc(&ctx.d_sink, 64));
+    const int blocks = sms * warps_per_subpartition;  // 128 threads = one warp per sub-partition per block
+    cudaEvent_t t0, t1;
+    CU(cudaEventCreate(&t0));
+    CU(cudaEventCreate(&t1));
+    cudaError_t e = lh::launch_issue_probe(variant, extra, iters / 8 + 1, blocks, ctx.d_sink, ctx.stream);  // warm-up
+    if (e == cudaErrorInvalidValue) {
+        cudaGetLastError();
+        return fail(LH_EINVAL, "lh_fp64_issue_probe: unknown variant %d / extra %d", variant, extra);
+    }
+    CU(e);
+    CU(cudaEventRecord(t0, ctx.stream));
+    CU(lh::launch_issue_probe(variant, extra, iters, blocks, ctx.d_sink, ctx.stream));
+    CU(cudaEventRecord(t1, ctx.stream));
+    CU(cudaEventSynchronize(t1));
+    ctx.launches += 2;
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, t0, t1));
+    cudaEventDestroy(t0);
+    cudaEventDestroy(t1);
+    *cycles_per_group = (double)ms * 1e-3 * (double)khz * 1e3 / ((double)iters * warps_per_subpartition);
+    return LH_OK;
+}
+
 const char *lh_version(void) { return "lh 0.1 sm_100a"; }
 
 }  // extern "C"

@@ -48,13 +48,15 @@ using SmemTables = MathTables;  // the atan / atanh reduction tables, staged per
 
 // ---- dPIE: core term minus cut term, merged ---------------------
 //   x' = c dx + s dy, y' = c dy - s dx, rho^2 = x'^2/p + y'^2/m, w_r = sqrt(r^2 + rho^2)
-//   P_r = o w_r + p r, Q_r = o w_r + m r, g_x = 2 sqrt(eps) x', g_y = 2 sqrt(eps) y'
+//   everything of sec. 5.2 divided by o = 1 - eps^2 so that each instruction has ONE uniform operand:
+//   P_r = w_r + (p/o) r, Q_r = w_r + (m/o) r, g_x = se x', g_y = se y', se = 2 sqrt(eps)/o
 //   alpha'_x = G atan ( g_x (P_t - P_c) / (P_c P_t + g_x^2) )
-//   alpha'_y = G atanh( g_y (Q_t - Q_c) / (Q_c Q_t - g_y^2) ),   G = T o / (2 sqrt(eps))
+//   alpha'_y = G atanh( g_y (Q_t - Q_c) / (Q_c Q_t - g_y^2) ),   G = T / se
 //   D_r = 2(1+eps^2) r^2 + 2 o r w_r + R^2,  f_r = 1/(w_r D_r)
 //   a11 + a22 += T (1/w_c - 1/w_t)
 //   a11 - a22 += T [ K (f_c rc^2 - f_t rt^2) - (dx^2 - dy^2)(f_c - f_t) ],  K  = -4 eps cos 2theta
 //   a12       += T [ K'(f_c rc^2 - f_t rt^2) -  dx dy       (f_c - f_t) ],  K' = -2 eps sin 2theta
+// The four reciprocals (reduced atan / atanh denominators, D_c, D_t) come from ONE seed (rcp4).
 template <bool GRAD, bool HESS>
 __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Acc &a, const SmemTables &tb) {
     const double dx = X - L.xc, dy = Y - L.yc;
@@ -65,19 +67,36 @@ __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Ac
     double wc, iwc, wt, iwt;
     rsqrt_sqrt(L.rc2 + rho2, wc, iwc);
     rsqrt_sqrt(L.rt2 + rho2, wt, iwt);
+    Reduced ra, rh;
+    double nx = 0.0, ny = 0.0, Dc = 1.0, Dt = 1.0, i1, i2, i3, i4;
     if (GRAD) {
-        const double Pc = fma(L.o, wc, L.prc), Pt = fma(L.o, wt, L.prt);
-        const double Qc = fma(L.o, wc, L.mrc), Qt = fma(L.o, wt, L.mrt);
+        const double Pc = wc + L.ac, Pt = wt + L.at;
+        const double Qc = wc + L.bc, Qt = wt + L.bt;
         const double gx = L.se * xp, gy = L.se * yp;
-        const double at = atan_nd(gx * (Pt - Pc), fma(gx, gx, Pc * Pt), tb.at);
-        const double ah = atanh_nd(gy * (Qt - Qc), fma(-gy, gy, Qc * Qt), tb.ah);
+        nx = gx * (Pt - Pc);
+        ny = gy * (Qt - Qc);
+        ra = atan_reduce(nx, fma(gx, gx, Pc * Pt), tb.at);
+        rh = atanh_reduce(ny, fma(-gy, gy, Qc * Qt), tb.ah);
+    }
+    if (HESS) {
+        const double R2 = xx + yy;
+        Dc = fma(L.orc2, wc, L.c0c + R2);
+        Dt = fma(L.ort2, wt, L.c0t + R2);
+    }
+    if (GRAD && HESS)
+        rcp4(ra.den, rh.den, Dc, Dt, i1, i2, i3, i4);
+    else if (GRAD)
+        rcp2(ra.den, rh.den, i1, i2);
+    else
+        rcp2(Dc, Dt, i3, i4);
+    if (GRAD) {
+        const double at = atan_finish(ra, i1, nx);
+        const double ah = atanh_finish(rh, i2, ny);
         a.ax = fma(L.cG, at, fma(-L.sG, ah, a.ax));
         a.ay = fma(L.sG, at, fma(L.cG, ah, a.ay));
     }
     if (HESS) {
-        const double R2 = xx + yy;
-        const double Dc = fma(L.orc2, wc, L.c0c + R2), Dt = fma(L.ort2, wt, L.c0t + R2);
-        const double fc = iwc * rcp(Dc), ft = iwt * rcp(Dt);
+        const double fc = iwc * i3, ft = iwt * i4;
         const double u = fma(fc, L.rc2, -(ft * L.rt2));
         const double Tv = L.T * (fc - ft);
         a.S = fma(L.T, iwc - iwt, a.S);
@@ -97,8 +116,13 @@ __device__ __forceinline__ void nsie_term(const LensK &L, double X, double Y, Ac
     double wc, iwc;
     rsqrt_sqrt(L.rc2 + rho2, wc, iwc);
     if (GRAD) {
-        const double at = atan_nd(L.se * xp, fma(L.o, wc, L.prc), tb.at);
-        const double ah = atanh_nd(L.se * yp, fma(L.o, wc, L.mrc), tb.ah);
+        const double nx = L.se * xp, ny = L.se * yp;
+        const Reduced ra = atan_reduce(nx, wc + L.ac, tb.at);
+        const Reduced rh = atanh_reduce(ny, wc + L.bc, tb.ah);
+        double i1, i2;
+        rcp2(ra.den, rh.den, i1, i2);
+        const double at = atan_finish(ra, i1, nx);
+        const double ah = atanh_finish(rh, i2, ny);
         a.ax = fma(L.cG, at, fma(-L.sG, ah, a.ax));
         a.ay = fma(L.sG, at, fma(L.cG, ah, a.ay));
     }
@@ -117,8 +141,7 @@ __device__ __forceinline__ void nsie_term(const LensK &L, double X, double Y, Ac
 // ---- CLS_EXTREME: dPIE / NSIE with eps > EXTREME_EPS (axis ratio < 0.02) ----------------------
 // Rare and slow on purpose: the two PIEMD terms are evaluated one by one with
 // IEEE sqrt / division and libdevice atan / atanh -- no table range limits, no merged-form
-// cancellation in d = Q_c Q_t - g_y^2 as u -> 1.  Not inlined: keeps its registers out of the
-// fast loops.  L.rt2 == 0 marks an NSIE (no cut term).
+// cancellation in d = Q_c Q_t - g_y^2 as u -> 1.  L.rt2 == 0 marks an NSIE (no cut term).
 template <bool GRAD, bool HESS>
 __device__ __forceinline__ void extreme_term(const LensK &L, double X, double Y, Acc &a) {
     const double dx = X - L.xc, dy = Y - L.yc;
@@ -133,13 +156,13 @@ __device__ __forceinline__ void extreme_term(const LensK &L, double X, double Y,
 #pragma unroll 1
     for (int term = 0; term < 2; ++term) {
         if (term == 1 && !cut) break;
-        const double r2 = term ? L.rt2 : L.rc2, pr = term ? L.prt : L.prc, mr = term ? L.mrt : L.mrc;
+        const double r2 = term ? L.rt2 : L.rc2, pr = term ? L.at : L.ac, mr = term ? L.bt : L.bc;
         const double or2 = term ? L.ort2 : L.orc2, c0 = term ? L.c0t : L.c0c;
         const double sg = term ? -1.0 : 1.0;
         const double w = sqrt(r2 + rho2);
         if (GRAD) {
-            jx += sg * atan(gx / fma(L.o, w, pr));
-            jy += sg * atanh(gy / fma(L.o, w, mr));
+            jx += sg * atan(gx / (w + pr));
+            jy += sg * atanh(gy / (w + mr));
         }
         if (HESS) {
             const double fr = 1.0 / (w * fma(or2, w, c0 + R2));

@@ -43,5 +43,6 @@ struct EvalJob {
 // Enqueues every launch of the job on `stream`; adds the number of kernels launched to *launches.
 cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launches);
 cudaError_t launch_dfma_probe(int iters, int blocks, double *sink, cudaStream_t stream);
+cudaError_t launch_issue_probe(int variant, int extra, int iters, int blocks, double *sink, cudaStream_t stream);  // lh_probe.cu
 
 }  // namespace lh

@@ -1,27 +1,31 @@
 // lh_math.cuh -- the FP64 primitives of the superposition kernel.
 //
 // The per-(pixel, lens) arithmetic of a dPIE needs two square roots with their
-// reciprocals, four reciprocals, one atan and one atanh.  libdevice spends ~190 FP64-pipe
-// instructions per evaluation on them; the B200 FP64 pipe issues one warp instruction
-// every two cycles per scheduler, so instruction count is the roofline.  These
-// replacements all follow one pattern:
+// reciprocals, four reciprocals, one atan and one atanh.  libdevice spends ~190 FP64
+// instructions per evaluation on them.  On the B200 an FP64 warp instruction holds the
+// dispatch port of its SM sub-partition for 2 cycles (3 when it reads three distinct vector
+// registers) and every other instruction for 1, so both counts matter.
+// These replacements all follow one pattern:
 //
 //   1. a 20-bit seed from the MUFU unit (MUFU.RCP64H / MUFU.RSQ64H: `rcp.approx.ftz.f64`,
-//      `rsqrt.approx.ftz.f64`; measured max relative error 9.9e-7 and 9.3e-7 on B200 --
-//      profiles/r01_mufu_probe.txt).  The XU pipe runs beside the FP64 pipe.
+//      `rsqrt.approx.ftz.f64`; relative error < 1e-6).
 //   2. ONE third-order correction in FMAs: error e -> O(e^3) ~ 1e-18, i.e. the result is
-//      good to a few ulp (measured 1.1e-16 / 1.7e-16).
+//      good to a few ulp.  Several reciprocals share one seed and one correction through
+//      the reciprocal of their product (rcp2 / rcp4).
 //   3. for atan / atanh: range reduction against a shared-memory table indexed by the
-//      approximate quotient (seed x numerator), with the quotient folded into the reduced
-//      argument so that each function costs ONE refined reciprocal:
-//        atan(n/d)  = atan(c) + atan( (n - c d)/(d + c n) )             c = i/128
-//        atanh(n/d) = atanh(c') + atanh( (n - c' d)/(d - c' n) ),  c' = (c-1)/(c+1) with
+//      exponent and the top 6 mantissa bits of the approximate quotient (seed x numerator),
+//      with the quotient folded into the reduced argument so that each function needs ONE
+//      refined reciprocal:
+//        atan(n/d)  = atan(c) + atan( (|n| - c d)/(d + c |n|) ),  c = |n|/d rounded to 6 bits
+//        atanh(n/d) = atanh(c') + atanh( (|n| - c' d)/(d - c' |n|) ),  c' = (c-1)/(c+1) with
 //                     c = (d+|n|)/(d-|n|) rounded to 6 mantissa bits (atanh c' = 1/2 ln c)
 //      and a two-term odd polynomial on |z| <= 2^-8 (truncation < 6e-16 relative).
+//      No branch, no swap of numerator and denominator: large quotients are large table
+//      indices.
 //
-// Every function is __host__ __device__ so that the same source can be exercised by the
-// CPU-only unit tests of the host logic; on the host the MUFU seeds are emulated by an
-// exact quotient truncated to 20 mantissa bits.
+// Every function is __host__ __device__ so that the CPU-only tests can pin the same source
+// (lh_math_host_eval in include/lh.h); on the host the MUFU seeds are emulated by an exact
+// quotient truncated to 20 mantissa bits.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -33,14 +37,17 @@
 
 namespace lh {
 
-constexpr int ATAN_N = 128;                 // atan table: c_i = i/128, i = 0..128
-constexpr int LN_OCTAVES = 16;              // atanh table: ratio c in [1, 2^16), 64 entries per octave
-constexpr int LN_PER_OCT = 64;
-constexpr int LN_N = LN_OCTAVES * LN_PER_OCT;
+// Both tables: entry 0 is the identity (c = 0 / c' = 0), entry 1 + 64 o + k is
+// c = 2^(o + O_MIN) (1 + k/64).
+constexpr int TAB_PER_OCT = 64;
+constexpr int ATAN_OCT_MIN = -8, ATAN_OCTAVES = 16;  // quotient in [2^-8, 2^8)
+constexpr int ATAN_N = ATAN_OCTAVES * TAB_PER_OCT + 1;
+constexpr int LN_OCTAVES = 16;                        // ratio (d+|n|)/(d-|n|) in [1, 2^16)
+constexpr int LN_N = LN_OCTAVES * TAB_PER_OCT + 1;
 
 struct MathTables {
-    double2 at[ATAN_N + 1];  // {c_i, atan(c_i)}
-    double2 ah[LN_N];        // {c'_j, atanh(c'_j)}, c'_j = (c_j-1)/(c_j+1), c_j = 2^(j/64) (linear inside an octave)
+    double2 at[ATAN_N];  // {c, atan c}
+    double2 ah[LN_N];    // {c', atanh c'}, c' = (c-1)/(c+1)
 };
 
 // ---- bit access -------------------------------------------------------------------------------
@@ -89,79 +96,118 @@ LH_HD double rcp(double x) {
     return fma(y, fma(e, e, e), y);
 }
 
+// 1/a and 1/b from one seed: r = 1/(a b), 1/a = r b, 1/b = r a.       6 FP64 + 1 MUFU
+LH_HD void rcp2(double a, double b, double &ia, double &ib) {
+    const double r = rcp(a * b);
+    ia = r * b;
+    ib = r * a;
+}
+
+// four reciprocals from one seed (product tree).                      12 FP64 + 1 MUFU
+// The product a b c d must stay inside the double range: lengths within ~1e+-35 (lh.h).
+LH_HD void rcp4(double a, double b, double c, double d, double &ia, double &ib, double &ic, double &id) {
+    const double ab = a * b, cd = c * d;
+    const double r = rcp(ab * cd);
+    const double rab = r * cd, rcd = r * ab;  // 1/(a b), 1/(c d)
+    ia = rab * b;
+    ib = rab * a;
+    ic = rcd * d;
+    id = rcd * c;
+}
+
 // w = sqrt(v) and iw = 1/sqrt(v), v > 0: seed + third-order step
-//   y (1 + e/2 + 3 e^2/8), e = 1 - v y^2.                              6 FP64 + 1 MUFU
+//   y (1 + e (1/2 + 3 e/8)), e = 1 - v y^2.                            6 FP64 + 1 MUFU
+// (the last FMA reads y twice: two distinct registers)
 LH_HD void rsqrt_sqrt(double v, double &w, double &iw) {
     const double y = rsq_seed(v);
     const double t = v * y;
     const double e = fma(-t, y, 1.0);
     const double c = fma(0.375, e, 0.5);
-    iw = fma(y * e, c, y);
+    iw = fma(y, c * e, y);
     w = v * iw;
 }
 
-// |x| and copysign as integer operations on the high word (ALU pipe, not the FP64 pipe)
+// |x| and copysign as integer operations on the high word (1 dispatch cycle, not 2)
 LH_HD double fabs_i(double x) { return mk64(hi32(x) & 0x7fffffff, lo32(x)); }
-LH_HD double copysign_i(double mag, double sgn) {
-    return mk64((hi32(mag) & 0x7fffffff) | (hi32(sgn) & (int)0x80000000), lo32(mag));
-}
-// a > b for two non-negative doubles: their bit patterns order like 64-bit integers
-LH_HD bool gt_nonneg(double a, double b) {
+// mag >= 0: one LOP3
+LH_HD double copysign_pos_i(double mag, double sgn) { return mk64(hi32(mag) | (hi32(sgn) & (int)0x80000000), lo32(mag)); }
+
+// Table index of a positive quotient q (approximate is enough): exponent and top 6 mantissa
+// bits, rounded to nearest; `bias` is the exponent of entry 1.  Everything below the table maps
+// to entry 0 (the identity), everything above (and NaN patterns) to the last entry.
+LH_HD unsigned quot_index(double q, int oct_min, int n) {
+    const int hr = hi32(q) + 0x2000;  // round to 6 mantissa bits (bit 13 is half a step)
+    const int j = (hr >> 14) - ((1023 + oct_min) << 6) + 1;
 #ifdef __CUDA_ARCH__
-    return __double_as_longlong(a) > __double_as_longlong(b);
+    return min((unsigned)max(j, 0), (unsigned)(n - 1));
 #else
-    int64_t x, y; std::memcpy(&x, &a, 8); std::memcpy(&y, &b, 8); return x > y;
+    return (unsigned)(j < 0 ? 0 : (j > n - 1 ? n - 1 : j));
 #endif
 }
 
-// atan(n/d) for d > 0 and any finite n.  Branch-free.                  12 FP64 + 2 MUFU
-LH_HD double atan_nd(double n, double d, const double2 *__restrict__ tab) {
+// ---- atan(n/d), d > 0, any finite n -----------------------------------------------------------
+// Split in two so that the caller can share the reciprocal of the reduced denominator with
+// other reciprocals (rcp2 / rcp4):
+//   atan_reduce: an = |n|, pick c, return num = an - c d and den = d + c an (> 0)   3 FP64 + 1 MUFU
+//   atan_finish: z = num/den given 1/den, atan c + z (1 - z^2/3 + z^4/5), sign of n 5 FP64
+struct Reduced {
+    double num, den, base;
+};
+LH_HD Reduced atan_reduce(double n, double d, const double2 *__restrict__ tab) {
     const double an = fabs_i(n);
-    const bool swap = gt_nonneg(an, d);
-    const double hi = swap ? an : d, lo = swap ? d : an;  // t = lo/hi in [0, 1]
-    // index: round(128 t) from the seed quotient, read from the low word after adding 1.5 * 2^45
-    const double kk = fma(lo, rcp_seed(hi), 52776558133248.0);
-    const unsigned i = min((unsigned)lo32(kk), (unsigned)ATAN_N);
-    const double2 ca = tab[i];  // {c, atan c}
-    const double num = fma(-ca.x, hi, lo), den = fma(ca.x, lo, hi);
-    const double z = num * rcp(den);  // |z| <= 2^-8
+    const double q0 = an * rcp_seed(d);  // |n|/d to 1e-6
+    const double2 ca = tab[quot_index(q0, ATAN_OCT_MIN, ATAN_N)];
+    return Reduced{fma(-ca.x, d, an), fma(ca.x, an, d), ca.y};
+}
+LH_HD double atan_finish(const Reduced &r, double iden, double n) {
+    const double z = r.num * iden;  // |z| <= 2^-8
     const double z2 = z * z;
     const double p = fma(z2, fma(z2, 0.2, -1.0 / 3.0), 1.0);
-    // swap: atan(t) = pi/2 - atan(1/t)  ->  res = base -+ (atan c + z p), one FMA either way
-    const double sg = swap ? -1.0 : 1.0, base = swap ? 1.5707963267948966 : 0.0;
-    const double r = fma(z, p, ca.y);
-    return copysign_i(fma(sg, r, base), n);
+    return copysign_pos_i(fma(z, p, r.base), n);
 }
 
-// atanh(n/d) for |n| < d with (d+|n|)/(d-|n|) < 2^16.  Branch-free.   13 FP64 + 2 MUFU
+// ---- atanh(n/d), |n| < d with (d+|n|)/(d-|n|) < 2^16 ------------------------------------------
 // The bin is chosen in the ratio domain q = (d+|n|)/(d-|n|) (so that the exponent of q does the
 // coarse part of the logarithm), the reduction is done in the u = n/d domain against
 // c' = (c-1)/(c+1), atanh(c') = 1/2 ln(c): both FMAs below see the exact n and d.
 // The host packer (lh_pack.cpp) routes every lens whose ellipticity could push q past the table
 // into the CLS_EXTREME class, which does not come through here; the index is clamped all the same.
-LH_HD double atanh_nd(double n, double d, const double2 *__restrict__ tab) {
-    const double an = fabs_i(n);                        // odd symmetry: q >= 1
-    const double a = d + an, b = d - an;
-    const double q0 = a * rcp_seed(b);                  // q to 1e-6
-    const int hr = hi32(q0) + 0x2000;                   // q rounded to 6 mantissa bits = c
-    const int j = max(0, min((hr >> 14) - (1023 << 6), LN_N - 1));
-    const double2 ca = tab[j];                          // {c', atanh c'}
-    const double num = fma(-ca.x, d, an), den = fma(-ca.x, an, d);
-    const double s = num * rcp(den);                    // |s| <= 2^-8
+//   atanh_reduce  5 FP64 + 1 MUFU      atanh_finish  5 FP64
+LH_HD Reduced atanh_reduce(double n, double d, const double2 *__restrict__ tab) {
+    const double an = fabs_i(n);  // odd symmetry: q >= 1
+    const double q0 = (d + an) * rcp_seed(d - an);
+    const double2 ca = tab[quot_index(q0, 0, LN_N)];
+    return Reduced{fma(-ca.x, d, an), fma(-ca.x, an, d), ca.y};
+}
+LH_HD double atanh_finish(const Reduced &r, double iden, double n) {
+    const double s = r.num * iden;  // |s| <= 2^-8
     const double s2 = s * s;
     const double p = fma(s2, fma(s2, 0.2, 1.0 / 3.0), 1.0);
-    return copysign_i(fma(s, p, ca.y), n);
+    return copysign_pos_i(fma(s, p, r.base), n);
 }
 
-// host: fill the tables (libm, correctly rounded enough: they are constants of the library)
+// Stand-alone forms (one reciprocal each)
+LH_HD double atan_nd(double n, double d, const double2 *__restrict__ tab) {
+    const Reduced r = atan_reduce(n, d, tab);
+    return atan_finish(r, rcp(r.den), n);
+}
+LH_HD double atanh_nd(double n, double d, const double2 *__restrict__ tab) {
+    const Reduced r = atanh_reduce(n, d, tab);
+    return atanh_finish(r, rcp(r.den), n);
+}
+
+// host: fill the tables (long-double libm: they are constants of the library)
 inline void fill_math_tables(MathTables &T) {
-    for (int i = 0; i <= ATAN_N; ++i) {
-        const double c = (double)i / ATAN_N;
-        T.at[i] = make_double2(c, (double)atanl((long double)c));
+    T.at[0] = make_double2(0.0, 0.0);
+    for (int j = 1; j < ATAN_N; ++j) {
+        const int e = (j - 1) / TAB_PER_OCT + ATAN_OCT_MIN, m = (j - 1) % TAB_PER_OCT;
+        const double c = std::ldexp(1.0 + (double)m / TAB_PER_OCT, e);
+        T.at[j] = make_double2(c, (double)atanl((long double)c));
     }
-    for (int j = 0; j < LN_N; ++j) {
-        const int e = j / LN_PER_OCT, m = j % LN_PER_OCT;
-        const long double c = std::ldexp(1.0L + (long double)m / LN_PER_OCT, e);
+    T.ah[0] = make_double2(0.0, 0.0);
+    for (int j = 1; j < LN_N; ++j) {
+        const int e = (j - 1) / TAB_PER_OCT, m = (j - 1) % TAB_PER_OCT;
+        const long double c = std::ldexp(1.0L + (long double)m / TAB_PER_OCT, e);
         const double cp = (double)((c - 1.0L) / (c + 1.0L));
         T.ah[j] = make_double2(cp, (double)atanhl((long double)cp));
     }

@@ -65,15 +65,16 @@ static void fill(const lh_lens &L, int cls, LensK &K) {
     K.rc2 = rc * rc;
     K.rt2 = rt * rt;
     K.o = o;
-    // The kernel evaluates G * atan(se x' .. ) with G = T o / se; at eps == 0 the limit is taken by a
-    // tiny stand-in (2^-500) for se: atan(u) = u exactly below 1e-8, so G * u is exact and (se x')^2 underflows to 0.
-    const double se = 2.0 * std::sqrt(eps);
+    // The kernel evaluates G * atan(se x' .. ) with G = T / se, se = 2 sqrt(eps) / o; at eps == 0 the limit is
+    // taken by a tiny stand-in (2^-500) for se: atan(u) = u exactly below 1e-8, so G * u is exact and
+    // (se x')^2 underflows to 0.
+    const double se = 2.0 * std::sqrt(eps) / o;
     K.se = (se > 0.0) ? se : 0x1p-500;
-    const double G = T * o / K.se;
-    K.prc = p * rc;
-    K.prt = p * rt;
-    K.mrc = m * rc;
-    K.mrt = m * rt;
+    const double G = T / K.se;
+    K.ac = p / o * rc;
+    K.at = p / o * rt;
+    K.bc = m / o * rc;
+    K.bt = m / o * rt;
     K.cG = K.c * G;
     K.sG = K.s * G;
     K.T = T;

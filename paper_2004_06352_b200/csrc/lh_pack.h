@@ -27,16 +27,18 @@ constexpr double EXTREME_EPS = 0.96;
 
 // Notation: eps = e/(1+sqrt(1-e^2)), o = 1-eps^2, p = (1+eps)^2,
 // m = (1-eps)^2, T = b0*rt/(rt-rc) (dPIE) or b0 (NSIE, SIS), c/s = cos/sin(theta).
+// The gradient constants are those of sec. 5.2 divided by o, so that every FP64 instruction of
+// the kernel takes at most ONE of these (uniform-register) fields.
 struct alignas(16) LensK {
     double xc, yc;      //  0  centre
     double c, s;        //  2  cos(theta), sin(theta)
     double ip, im;      //  4  1/p, 1/m              -> rho^2 = ip x'^2 + im y'^2
     double rc2, rt2;    //  6  rcore^2, rcut^2       -> w_r = sqrt(r^2 + rho^2); rt2 = 0 marks an NSIE in CLS_EXTREME
-    double o, se;       //  8  1-eps^2; 2 sqrt(eps), replaced by 2^-500 when eps == 0
-    double prc, prt;    // 10  p*rcore, p*rcut       -> P_r = o w_r + p r
-    double mrc, mrt;    // 12  m*rcore, m*rcut       -> Q_r = o w_r + m r
-    double cG, sG;      // 14  cos, sin(theta) * G,  G = T o / se
-    double T, eps;      // 16  T; eps (read by the CLS_EXTREME path only)
+    double o, se;       //  8  1-eps^2; 2 sqrt(eps)/o, replaced by 2^-500 when eps == 0
+    double ac, at;      // 10  (p/o) rcore, (p/o) rcut   -> P_r = w_r + a_r
+    double bc, bt;      // 12  (m/o) rcore, (m/o) rcut   -> Q_r = w_r + b_r
+    double cG, sG;      // 14  cos, sin(theta) * G,  G = T / se
+    double T, eps;      // 16  T; eps (diagnostic)
     double orc2, ort2;  // 18  2 o rcore, 2 o rcut   -> D_r = c0_r + R^2 + (2 o r) w_r
     double c0c, c0t;    // 20  2 (1+eps^2) r^2
     double KT, K2T;     // 22  -4 eps cos(2 theta) T, -2 eps sin(2 theta) T

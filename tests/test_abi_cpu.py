@@ -79,11 +79,11 @@ def test_pack_constants():
     eps = 1.0 / 3.0  # e-hat 0.6 <-> eps 1/3 (reading 8c-2)
     o, p, m = 1 - eps ** 2, (1 + eps) ** 2, (1 - eps) ** 2
     T = 3.0 * 40.0 / (40.0 - 0.25)
-    se = 2 * math.sqrt(eps)
-    G = T * o / se
-    want = [1.5, -2.0, math.cos(0.3), math.sin(0.3), 1 / p, 1 / m, 0.25 ** 2, 40.0 ** 2, o, se, p * 0.25,
-            p * 40.0, m * 0.25, m * 40.0, math.cos(0.3) * G, math.sin(0.3) * G, T]
-    assert np.allclose(k[:17], want, rtol=1e-15, atol=0)
+    se = 2 * math.sqrt(eps) / o  # sec. 5.2 divided by o: one uniform operand per instruction
+    G = T / se
+    want = [1.5, -2.0, math.cos(0.3), math.sin(0.3), 1 / p, 1 / m, 0.25 ** 2, 40.0 ** 2, o, se, p / o * 0.25,
+            p / o * 40.0, m / o * 0.25, m / o * 40.0, math.cos(0.3) * G, math.sin(0.3) * G, T]
+    assert np.allclose(k[:17], want, rtol=4e-16, atol=0)
     assert np.allclose(k[18:], [2 * o * 0.25, 2 * o * 40.0, 2 * (1 + eps ** 2) * 0.0625, 2 * (1 + eps ** 2) * 1600,
                                 -4 * eps * math.cos(0.6) * T, -2 * eps * math.sin(0.6) * T], rtol=1e-15)
     # circular lens: the 2 sqrt(eps) -> 0 limit is taken with a tiny stand-in, G se = T o stays exact
