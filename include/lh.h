@@ -150,7 +150,7 @@ int lh_fp64_peak_probe(int iters, double *flops_per_s, double *seconds);
  * device; on the host the 20-bit MUFU seeds are emulated by truncated exact quotients), so that
  * CPU-only tests can pin them against libm / arbitrary precision.  out[k] = fn(a[k], b[k]):
  *   fn 0  1/a            1  sqrt(a)        2  1/sqrt(a)
- *      3  atan(a/b), b > 0                 4  atanh(a/b), |a| < b, (b+|a|)/(b-|a|) < 2^16
+ *      3  atan(a/b), b > 0                 4  atanh(a/b), |a| < b, 1 - |a|/b > 2^-16
  *      5  1/a via the shared-seed pair (a, b)     6  1/a via the shared-seed quadruple (a, b, a+b, 2b)
  * No CUDA call is made.  LH_EINVAL for an unknown fn or a NULL pointer (b may be NULL for fn 0-2). */
 int lh_math_host_eval(int fn, const double *a, const double *b, size_t n, double *out);

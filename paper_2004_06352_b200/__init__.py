@@ -44,13 +44,13 @@ _lib = None
 
 
 def library_path() -> str:
-    return _build.LIB
+    return os.environ.get("LH_LIBRARY", _build.LIB)
 
 
 def _load():
     global _lib
     if _lib is None:
-        path = _build.LIB
+        path = os.environ.get("LH_LIBRARY", _build.LIB)  # LH_LIBRARY: another build of the same library
         if not os.path.exists(path):
             raise ImportError(
                 f"{path} is missing: build it with `python -m paper_2004_06352_b200._build` "

@@ -47,16 +47,15 @@ struct Acc {
 using SmemTables = MathTables;  // the atan / atanh reduction tables, staged per CTA
 
 // ---- dPIE: core term minus cut term, merged ---------------------
-//   x' = c dx + s dy, y' = c dy - s dx, rho^2 = x'^2/p + y'^2/m, w_r = sqrt(r^2 + rho^2)
-//   everything of sec. 5.2 divided by o = 1 - eps^2 so that each instruction has ONE uniform operand:
-//   P_r = w_r + (p/o) r, Q_r = w_r + (m/o) r, g_x = se x', g_y = se y', se = 2 sqrt(eps)/o
-//   alpha'_x = G atan ( g_x (P_t - P_c) / (P_c P_t + g_x^2) )
-//   alpha'_y = G atanh( g_y (Q_t - Q_c) / (Q_c Q_t - g_y^2) ),   G = T / se
-//   D_r = 2(1+eps^2) r^2 + 2 o r w_r + R^2,  f_r = 1/(w_r D_r)
-//   a11 + a22 += T (1/w_c - 1/w_t)
-//   a11 - a22 += T [ K (f_c rc^2 - f_t rt^2) - (dx^2 - dy^2)(f_c - f_t) ],  K  = -4 eps cos 2theta
-//   a12       += T [ K'(f_c rc^2 - f_t rt^2) -  dx dy       (f_c - f_t) ],  K' = -2 eps sin 2theta
-// The four reciprocals (reduced atan / atanh denominators, D_c, D_t) come from ONE seed (rcp4).
+// Lens frame scaled by k = o / (2 sqrt eps):  x' = c dx + s dy, y' = c dy - s dx,
+//   w^_r = k w_r = sqrt(k^2 r^2 + k^2 rho^2),  P^_r = w^_r + (p/sg) r,  Q^_r = w^_r + (m/sg) r
+//   alpha'_x = G atan ( x' (P^_t - P^_c) / (P^_c P^_t + x'^2) )
+//   alpha'_y = G atanh( y' (Q^_t - Q^_c) / (Q^_c Q^_t - y'^2) ),         G = T k
+//   D_r = (sg^2/p) (P^_r^2 + x'^2),  f^_r = 1 / (w^_r (P^_r^2 + x'^2)) = f_r / (k p / sg^2)
+//   a11 + a22 += G  (1/w^_c - 1/w^_t)
+//   a11 - a22 += TF [ K (f^_c rc^2 - f^_t rt^2) - (dx^2 - dy^2)(f^_c - f^_t) ],  K  = -4 eps cos 2theta
+//   a12       += TF [ K'(f^_c rc^2 - f^_t rt^2) -  dx dy       (f^_c - f^_t) ],  K' = -2 eps sin 2theta
+// The four reciprocals (reduced atan / atanh denominators, D^_c, D^_t) come from ONE seed (rcp4).
 template <bool GRAD, bool HESS>
 __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Acc &a, const SmemTables &tb) {
     const double dx = X - L.xc, dy = Y - L.yc;
@@ -67,21 +66,19 @@ __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Ac
     double wc, iwc, wt, iwt;
     rsqrt_sqrt(L.rc2 + rho2, wc, iwc);
     rsqrt_sqrt(L.rt2 + rho2, wt, iwt);
+    const double Pc = wc + L.ac, Pt = wt + L.at;
     Reduced ra, rh;
     double nx = 0.0, ny = 0.0, Dc = 1.0, Dt = 1.0, i1, i2, i3, i4;
     if (GRAD) {
-        const double Pc = wc + L.ac, Pt = wt + L.at;
         const double Qc = wc + L.bc, Qt = wt + L.bt;
-        const double gx = L.se * xp, gy = L.se * yp;
-        nx = gx * (Pt - Pc);
-        ny = gy * (Qt - Qc);
-        ra = atan_reduce(nx, fma(gx, gx, Pc * Pt), tb.at);
-        rh = atanh_reduce(ny, fma(-gy, gy, Qc * Qt), tb.ah);
+        nx = xp * (Pt - Pc);
+        ny = yp * (Qt - Qc);
+        ra = atan_reduce(nx, fma(xp, xp, Pc * Pt), tb.at);
+        rh = atanh_reduce(ny, fma(-yp, yp, Qc * Qt), tb.ah);
     }
     if (HESS) {
-        const double R2 = xx + yy;
-        Dc = fma(L.orc2, wc, L.c0c + R2);
-        Dt = fma(L.ort2, wt, L.c0t + R2);
+        Dc = fma(Pc, Pc, xx);
+        Dt = fma(Pt, Pt, xx);
     }
     if (GRAD && HESS)
         rcp4(ra.den, rh.den, Dc, Dt, i1, i2, i3, i4);
@@ -97,11 +94,11 @@ __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Ac
     }
     if (HESS) {
         const double fc = iwc * i3, ft = iwt * i4;
-        const double u = fma(fc, L.rc2, -(ft * L.rt2));
-        const double Tv = L.T * (fc - ft);
-        a.S = fma(L.T, iwc - iwt, a.S);
-        a.Dl = fma(L.KT, u, fma(-fma(dx, dx, -(dy * dy)), Tv, a.Dl));
-        a.a12 = fma(L.K2T, u, fma(-(dx * dy), Tv, a.a12));
+        const double u = fma(fc, L.r2c, -(ft * L.r2t));
+        const double Tv = L.TF * (fc - ft);
+        a.S = fma(L.G, iwc - iwt, a.S);
+        a.Dl = fma(L.KTF, u, fma(-fma(dx, dx, -(dy * dy)), Tv, a.Dl));
+        a.a12 = fma(L.K2TF, u, fma(-(dx * dy), Tv, a.a12));
     }
 }
 
@@ -115,33 +112,32 @@ __device__ __forceinline__ void nsie_term(const LensK &L, double X, double Y, Ac
     const double rho2 = fma(L.ip, xx, L.im * yy);
     double wc, iwc;
     rsqrt_sqrt(L.rc2 + rho2, wc, iwc);
+    const double Pc = wc + L.ac;
     if (GRAD) {
-        const double nx = L.se * xp, ny = L.se * yp;
-        const Reduced ra = atan_reduce(nx, wc + L.ac, tb.at);
-        const Reduced rh = atanh_reduce(ny, wc + L.bc, tb.ah);
+        const Reduced ra = atan_reduce(xp, Pc, tb.at);
+        const Reduced rh = atanh_reduce(yp, wc + L.bc, tb.ah);
         double i1, i2;
         rcp2(ra.den, rh.den, i1, i2);
-        const double at = atan_finish(ra, i1, nx);
-        const double ah = atanh_finish(rh, i2, ny);
+        const double at = atan_finish(ra, i1, xp);
+        const double ah = atanh_finish(rh, i2, yp);
         a.ax = fma(L.cG, at, fma(-L.sG, ah, a.ax));
         a.ay = fma(L.sG, at, fma(L.cG, ah, a.ay));
     }
     if (HESS) {
-        const double R2 = xx + yy;
-        const double Dc = fma(L.orc2, wc, L.c0c + R2);
-        const double fc = iwc * rcp(Dc);
-        const double u = fc * L.rc2;
-        const double Tv = L.T * fc;
-        a.S = fma(L.T, iwc, a.S);
-        a.Dl = fma(L.KT, u, fma(-fma(dx, dx, -(dy * dy)), Tv, a.Dl));
-        a.a12 = fma(L.K2T, u, fma(-(dx * dy), Tv, a.a12));
+        const double fc = iwc * rcp(fma(Pc, Pc, xx));
+        const double u = fc * L.r2c;
+        const double Tv = L.TF * fc;
+        a.S = fma(L.G, iwc, a.S);
+        a.Dl = fma(L.KTF, u, fma(-fma(dx, dx, -(dy * dy)), Tv, a.Dl));
+        a.a12 = fma(L.K2TF, u, fma(-(dx * dy), Tv, a.a12));
     }
 }
 
 // ---- CLS_EXTREME: dPIE / NSIE with eps > EXTREME_EPS (axis ratio < 0.02) ----------------------
-// Rare and slow on purpose: the two PIEMD terms are evaluated one by one with
-// IEEE sqrt / division and libdevice atan / atanh -- no table range limits, no merged-form
-// cancellation in d = Q_c Q_t - g_y^2 as u -> 1.  L.rt2 == 0 marks an NSIE (no cut term).
+// Rare and slow on purpose: the two PIEMD terms are evaluated one by one (same
+// scaled frame) with IEEE sqrt / division and libdevice atan / atanh -- no table range limits, no
+// merged-form cancellation in Q^_c Q^_t - y'^2 as the atanh argument -> 1.  L.rt2 == 0 marks an
+// NSIE (no cut term).
 template <bool GRAD, bool HESS>
 __device__ __forceinline__ void extreme_term(const LensK &L, double X, double Y, Acc &a) {
     const double dx = X - L.xc, dy = Y - L.yc;
@@ -149,25 +145,24 @@ __device__ __forceinline__ void extreme_term(const LensK &L, double X, double Y,
     const double yp = fma(-L.s, dx, L.c * dy);
     const double xx = xp * xp, yy = yp * yp;
     const double rho2 = fma(L.ip, xx, L.im * yy);
-    const double R2 = xx + yy;
-    const double gx = L.se * xp, gy = L.se * yp;
     const bool cut = L.rt2 > 0.0;
     double jx = 0.0, jy = 0.0, S = 0.0, u = 0.0, f = 0.0;
 #pragma unroll 1
     for (int term = 0; term < 2; ++term) {
         if (term == 1 && !cut) break;
-        const double r2 = term ? L.rt2 : L.rc2, pr = term ? L.at : L.ac, mr = term ? L.bt : L.bc;
-        const double or2 = term ? L.ort2 : L.orc2, c0 = term ? L.c0t : L.c0c;
+        const double r2 = term ? L.rt2 : L.rc2, ar = term ? L.at : L.ac, br = term ? L.bt : L.bc;
+        const double r2true = term ? L.r2t : L.r2c;
         const double sg = term ? -1.0 : 1.0;
         const double w = sqrt(r2 + rho2);
+        const double P = w + ar;
         if (GRAD) {
-            jx += sg * atan(gx / (w + pr));
-            jy += sg * atanh(gy / (w + mr));
+            jx += sg * atan(xp / P);
+            jy += sg * atanh(yp / (w + br));
         }
         if (HESS) {
-            const double fr = 1.0 / (w * fma(or2, w, c0 + R2));
+            const double fr = 1.0 / (w * fma(P, P, xx));
             S += sg / w;
-            u += sg * fr * r2;
+            u += sg * fr * r2true;
             f += sg * fr;
         }
     }
@@ -176,10 +171,10 @@ __device__ __forceinline__ void extreme_term(const LensK &L, double X, double Y,
         a.ay = fma(L.sG, jx, fma(L.cG, jy, a.ay));
     }
     if (HESS) {
-        const double Tv = L.T * f;
-        a.S = fma(L.T, S, a.S);
-        a.Dl = fma(L.KT, u, fma(-fma(dx, dx, -(dy * dy)), Tv, a.Dl));
-        a.a12 = fma(L.K2T, u, fma(-(dx * dy), Tv, a.a12));
+        const double Tv = L.TF * f;
+        a.S = fma(L.G, S, a.S);
+        a.Dl = fma(L.KTF, u, fma(-fma(dx, dx, -(dy * dy)), Tv, a.Dl));
+        a.a12 = fma(L.K2TF, u, fma(-(dx * dy), Tv, a.a12));
     }
 }
 
@@ -191,7 +186,7 @@ __device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc
     double R, iR;
     rsqrt_sqrt(R2, R, iR);
     if (!(R2 > 0.0)) iR = 0.0;
-    const double g = L.T * iR;
+    const double g = L.G * iR;
     if (GRAD) {
         a.ax = fma(g, dx, a.ax);
         a.ay = fma(g, dy, a.ay);

@@ -17,8 +17,8 @@
 //      with the quotient folded into the reduced argument so that each function needs ONE
 //      refined reciprocal:
 //        atan(n/d)  = atan(c) + atan( (|n| - c d)/(d + c |n|) ),  c = |n|/d rounded to 6 bits
-//        atanh(n/d) = atanh(c') + atanh( (|n| - c' d)/(d - c' |n|) ),  c' = (c-1)/(c+1) with
-//                     c = (d+|n|)/(d-|n|) rounded to 6 mantissa bits (atanh c' = 1/2 ln c)
+//        atanh(n/d) = atanh(c') + atanh( (|n| - c' d)/(d - c' |n|) ),  c' = 1 - t_c with
+//                     t_c = 1 - |n|/d rounded to 6 mantissa bits
 //      and a two-term odd polynomial on |z| <= 2^-8 (truncation < 6e-16 relative).
 //      No branch, no swap of numerator and denominator: large quotients are large table
 //      indices.
@@ -42,12 +42,12 @@ namespace lh {
 constexpr int TAB_PER_OCT = 64;
 constexpr int ATAN_OCT_MIN = -8, ATAN_OCTAVES = 16;  // quotient in [2^-8, 2^8)
 constexpr int ATAN_N = ATAN_OCTAVES * TAB_PER_OCT + 1;
-constexpr int LN_OCTAVES = 16;                        // ratio (d+|n|)/(d-|n|) in [1, 2^16)
+constexpr int LN_OCTAVES = 16;                        // t = 1 - |n|/d in (2^-16, 1]
 constexpr int LN_N = LN_OCTAVES * TAB_PER_OCT + 1;
 
 struct MathTables {
     double2 at[ATAN_N];  // {c, atan c}
-    double2 ah[LN_N];    // {c', atanh c'}, c' = (c-1)/(c+1)
+    double2 ah[LN_N];    // {c', atanh c'}, c' = 1 - t_c
 };
 
 // ---- bit access -------------------------------------------------------------------------------
@@ -116,15 +116,16 @@ LH_HD void rcp4(double a, double b, double c, double d, double &ia, double &ib, 
 }
 
 // w = sqrt(v) and iw = 1/sqrt(v), v > 0: seed + third-order step
-//   y (1 + e (1/2 + 3 e/8)), e = 1 - v y^2.                            6 FP64 + 1 MUFU
-// (the last FMA reads y twice: two distinct registers)
+//   (1 + h) y and (1 + h) v y,  h = e (1/2 + 3 e/8), e = 1 - v y^2.     6 FP64 + 1 MUFU
+// (both closing FMAs read one register twice: two distinct registers each; a caller that
+// drops iw pays 5)
 LH_HD void rsqrt_sqrt(double v, double &w, double &iw) {
     const double y = rsq_seed(v);
     const double t = v * y;
     const double e = fma(-t, y, 1.0);
-    const double c = fma(0.375, e, 0.5);
-    iw = fma(y, c * e, y);
-    w = v * iw;
+    const double h = fma(0.375, e, 0.5) * e;
+    iw = fma(y, h, y);
+    w = fma(t, h, t);
 }
 
 // |x| and copysign as integer operations on the high word (1 dispatch cycle, not 2)
@@ -138,6 +139,19 @@ LH_HD double copysign_pos_i(double mag, double sgn) { return mk64(hi32(mag) | (h
 LH_HD unsigned quot_index(double q, int oct_min, int n) {
     const int hr = hi32(q) + 0x2000;  // round to 6 mantissa bits (bit 13 is half a step)
     const int j = (hr >> 14) - ((1023 + oct_min) << 6) + 1;
+#ifdef __CUDA_ARCH__
+    return min((unsigned)max(j, 0), (unsigned)(n - 1));
+#else
+    return (unsigned)(j < 0 ? 0 : (j > n - 1 ? n - 1 : j));
+#endif
+}
+
+// Table index of t in (0, 1] counted DOWN from 1: entry 0 is t = 1 (c' = 0), entry 64 o + k,
+// k = 0..63, is t_c = 2^-(o+1) (2 - k/64) ... i.e. the exponent/6-bit-mantissa code of t
+// subtracted from that of 1.0.  t above 1 (rounding) maps to entry 0, t below the table to the last.
+LH_HD unsigned quot_index_down(double t, int n) {
+    const int hr = hi32(t) + 0x2000;
+    const int j = (1023 << 6) - (hr >> 14);
 #ifdef __CUDA_ARCH__
     return min((unsigned)max(j, 0), (unsigned)(n - 1));
 #else
@@ -166,21 +180,23 @@ LH_HD double atan_finish(const Reduced &r, double iden, double n) {
     return copysign_pos_i(fma(z, p, r.base), n);
 }
 
-// ---- atanh(n/d), |n| < d with (d+|n|)/(d-|n|) < 2^16 ------------------------------------------
-// The bin is chosen in the ratio domain q = (d+|n|)/(d-|n|) (so that the exponent of q does the
-// coarse part of the logarithm), the reduction is done in the u = n/d domain against
-// c' = (c-1)/(c+1), atanh(c') = 1/2 ln(c): both FMAs below see the exact n and d.
-// The host packer (lh_pack.cpp) routes every lens whose ellipticity could push q past the table
-// into the CLS_EXTREME class, which does not come through here; the index is clamped all the same.
-//   atanh_reduce  5 FP64 + 1 MUFU      atanh_finish  5 FP64
+// ---- atanh(n/d), 0 <= |n| < d with 1 - |n|/d > 2^-16 -----------------------------------------
+// u = |n|/d; the bin is chosen on t = 1 - u = (d-|n|)/d, whose exponent follows the singularity
+// of atanh at u = 1: bins are t_c = 2^-e (1 + k/64), c' = 1 - t_c, so that the reduced argument
+//   s = (|n| - c' d)/(d - c' |n|) = (u - c')/(1 - c' u)
+// stays below 2^-7.5 everywhere (|u - c'| <= t/128 and 1 - c'u >= 1 - u^2 ~ 2t near u = 1).
+// Both FMAs see the exact n and d.  The host packer (lh_pack.cpp) routes every lens whose
+// ellipticity could push u past the table into the CLS_EXTREME class, which does not come
+// through here; the index is clamped all the same.
+//   atanh_reduce  4 FP64 + 1 MUFU      atanh_finish  5 FP64
 LH_HD Reduced atanh_reduce(double n, double d, const double2 *__restrict__ tab) {
-    const double an = fabs_i(n);  // odd symmetry: q >= 1
-    const double q0 = (d + an) * rcp_seed(d - an);
-    const double2 ca = tab[quot_index(q0, 0, LN_N)];
+    const double an = fabs_i(n);
+    const double t0 = (d - an) * rcp_seed(d);  // 1 - u to 1e-6 relative
+    const double2 ca = tab[quot_index_down(t0, LN_N)];
     return Reduced{fma(-ca.x, d, an), fma(-ca.x, an, d), ca.y};
 }
 LH_HD double atanh_finish(const Reduced &r, double iden, double n) {
-    const double s = r.num * iden;  // |s| <= 2^-8
+    const double s = r.num * iden;
     const double s2 = s * s;
     const double p = fma(s2, fma(s2, 0.2, 1.0 / 3.0), 1.0);
     return copysign_pos_i(fma(s, p, r.base), n);
@@ -204,11 +220,11 @@ inline void fill_math_tables(MathTables &T) {
         const double c = std::ldexp(1.0 + (double)m / TAB_PER_OCT, e);
         T.at[j] = make_double2(c, (double)atanl((long double)c));
     }
-    T.ah[0] = make_double2(0.0, 0.0);
-    for (int j = 1; j < LN_N; ++j) {
-        const int e = (j - 1) / TAB_PER_OCT, m = (j - 1) % TAB_PER_OCT;
-        const long double c = std::ldexp(1.0L + (long double)m / TAB_PER_OCT, e);
-        const double cp = (double)((c - 1.0L) / (c + 1.0L));
+    // entry j <-> code(1.0) - j: j = 64 o + k, k = 1..64  ->  t_c = 2^-(o+1) (2 - k/64)  (k = 64: 2^-(o+1))
+    for (int j = 0; j < LN_N; ++j) {
+        const int code = (1023 << 6) - j;  // exponent field and 6 mantissa bits of t_c
+        const double tc = std::ldexp(1.0 + (double)(code & 63) / TAB_PER_OCT, (code >> 6) - 1023);
+        const double cp = 1.0 - tc;  // exact
         T.ah[j] = make_double2(cp, (double)atanhl((long double)cp));
     }
 }

@@ -46,45 +46,45 @@ static void fill(const lh_lens &L, int cls, LensK &K) {
     K.xc = L.x;
     K.yc = L.y;
     if (cls == CLS_SIS) {
-        K.T = L.b0;
+        K.G = K.T = L.b0;
         K.c = 1.0;
         return;
     }
     const double e = L.ellipticity;
-    const double eps = e / (1.0 + std::sqrt(1.0 - e * e));  // reading 8c-2
+    const double eps = e / (1.0 + std::sqrt(1.0 - e * e));  // reading R2
     const double o = 1.0 - eps * eps, p = (1.0 + eps) * (1.0 + eps), m = (1.0 - eps) * (1.0 - eps);
     const double rc = L.rcore;
     const bool cut = (L.type == LH_DPIE);
     const double rt = cut ? L.rcut : 0.0;
     const double T = cut ? L.b0 * rt / (rt - rc) : L.b0;
+    // eps -> 0 is taken by never letting 2 sqrt(eps) fall below 2^-64: the scaled frame then makes x'^2
+    // vanish against P^_c P^_t exactly (atan(u) = u below 1e-8) and every product stays far inside the
+    // double range; the deviation from the true tiny eps is O(eps) < 2^-130 relative.
+    const double sg = std::fmax(2.0 * std::sqrt(eps), 0x1p-64);
+    const double k = o / sg;
     const double c2 = std::cos(2.0 * L.theta), s2 = std::sin(2.0 * L.theta);
     K.c = std::cos(L.theta);
     K.s = std::sin(L.theta);
-    K.ip = 1.0 / p;
-    K.im = 1.0 / m;
-    K.rc2 = rc * rc;
-    K.rt2 = rt * rt;
-    K.o = o;
-    // The kernel evaluates G * atan(se x' .. ) with G = T / se, se = 2 sqrt(eps) / o; at eps == 0 the limit is
-    // taken by a tiny stand-in (2^-500) for se: atan(u) = u exactly below 1e-8, so G * u is exact and
-    // (se x')^2 underflows to 0.
-    const double se = 2.0 * std::sqrt(eps) / o;
-    K.se = (se > 0.0) ? se : 0x1p-500;
-    const double G = T / K.se;
-    K.ac = p / o * rc;
-    K.at = p / o * rt;
-    K.bc = m / o * rc;
-    K.bt = m / o * rt;
-    K.cG = K.c * G;
-    K.sG = K.s * G;
-    K.T = T;
+    K.ip = k * k / p;
+    K.im = k * k / m;
+    K.rc2 = k * k * rc * rc;
+    K.rt2 = k * k * rt * rt;
+    K.ac = p / sg * rc;
+    K.at = p / sg * rt;
+    K.bc = m / sg * rc;
+    K.bt = m / sg * rt;
+    K.G = T * k;
+    K.cG = K.c * K.G;
+    K.sG = K.s * K.G;
+    K.TF = T * k * p / (sg * sg);
+    K.r2c = rc * rc;
+    K.r2t = rt * rt;
+    K.KTF = -4.0 * eps * c2 * K.TF;
+    K.K2TF = -2.0 * eps * s2 * K.TF;
     K.eps = eps;
-    K.orc2 = 2.0 * o * rc;
-    K.ort2 = 2.0 * o * rt;
-    K.c0c = 2.0 * (1.0 + eps * eps) * rc * rc;
-    K.c0t = 2.0 * (1.0 + eps * eps) * rt * rt;
-    K.KT = -4.0 * eps * c2 * T;
-    K.K2T = -2.0 * eps * s2 * T;
+    K.o = o;
+    K.sg = sg;
+    K.T = T;
 }
 
 int pack_model(const void *records, int n, LensK *out, ModelRanges *ranges, char *err, int errlen, int model) {

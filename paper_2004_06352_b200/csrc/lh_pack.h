@@ -25,23 +25,25 @@ enum LensClass : int {
 // of the atanh table: eps = 0.96 <-> e-hat = 0.99917 <-> axis ratio q = 0.0204 <-> ratio < 9700.
 constexpr double EXTREME_EPS = 0.96;
 
-// Notation: eps = e/(1+sqrt(1-e^2)), o = 1-eps^2, p = (1+eps)^2,
-// m = (1-eps)^2, T = b0*rt/(rt-rc) (dPIE) or b0 (NSIE, SIS), c/s = cos/sin(theta).
-// The gradient constants are those of sec. 5.2 divided by o, so that every FP64 instruction of
-// the kernel takes at most ONE of these (uniform-register) fields.
+// Notation: eps = e/(1+sqrt(1-e^2)), o = 1-eps^2, p = (1+eps)^2, m = (1-eps)^2,
+// sg = 2 sqrt(eps) (never below 2^-64, which takes the circular limit), k = o/sg,
+// T = b0*rt/(rt-rc) (dPIE) or b0 (NSIE, SIS), c/s = cos/sin(theta).
+// All lengths of the lens frame are carried scaled by k (w^ = k w), which removes the
+// 2 sqrt(eps) factors from the atan / atanh arguments (sec. 5.2) and turns D_r into
+// (sg^2/p)(P^_r^2 + x'^2) (sec. 5.3); every FP64 instruction of the kernel takes at most ONE field.
 struct alignas(16) LensK {
     double xc, yc;      //  0  centre
     double c, s;        //  2  cos(theta), sin(theta)
-    double ip, im;      //  4  1/p, 1/m              -> rho^2 = ip x'^2 + im y'^2
-    double rc2, rt2;    //  6  rcore^2, rcut^2       -> w_r = sqrt(r^2 + rho^2); rt2 = 0 marks an NSIE in CLS_EXTREME
-    double o, se;       //  8  1-eps^2; 2 sqrt(eps)/o, replaced by 2^-500 when eps == 0
-    double ac, at;      // 10  (p/o) rcore, (p/o) rcut   -> P_r = w_r + a_r
-    double bc, bt;      // 12  (m/o) rcore, (m/o) rcut   -> Q_r = w_r + b_r
-    double cG, sG;      // 14  cos, sin(theta) * G,  G = T / se
-    double T, eps;      // 16  T; eps (diagnostic)
-    double orc2, ort2;  // 18  2 o rcore, 2 o rcut   -> D_r = c0_r + R^2 + (2 o r) w_r
-    double c0c, c0t;    // 20  2 (1+eps^2) r^2
-    double KT, K2T;     // 22  -4 eps cos(2 theta) T, -2 eps sin(2 theta) T
+    double ip, im;      //  4  k^2/p, k^2/m          -> rho^^2 = ip x'^2 + im y'^2
+    double rc2, rt2;    //  6  k^2 rcore^2, k^2 rcut^2 -> w^_r = sqrt(r2 + rho^^2); rt2 = 0 marks an NSIE in CLS_EXTREME
+    double ac, at;      //  8  (p/sg) rcore, (p/sg) rcut -> P^_r = w^_r + a_r
+    double bc, bt;      // 10  (m/sg) rcore, (m/sg) rcut -> Q^_r = w^_r + b_r
+    double cG, sG;      // 12  cos, sin(theta) * G
+    double G, TF;       // 14  G = T k (also the weight of 1/w^_c - 1/w^_t; SIS: b0);  TF = T k p / sg^2 (weight of f^_r)
+    double r2c, r2t;    // 16  rcore^2, rcut^2 (unscaled)
+    double KTF, K2TF;   // 18  -4 eps cos(2 theta) TF, -2 eps sin(2 theta) TF
+    double eps, o;      // 20  diagnostic
+    double sg, T;       // 22  diagnostic
 };
 static_assert(sizeof(LensK) == 24 * 8, "LensK is 24 doubles");
 constexpr int LENSK_DOUBLES = sizeof(LensK) / 8;

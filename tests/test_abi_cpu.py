@@ -66,29 +66,33 @@ def test_pack_routes_extreme_ellipticity_to_its_own_class():
     t, begin = lh.lh_pack_model(L)
     assert list(begin) == [0, 1, 2, 3, 5]
     assert list(t[:, 0]) == [0.0, 4.0, 3.0, 1.0, 2.0]
-    assert t[3, 7] == 100.0 and t[4, 7] == 0.0  # rt^2; 0 marks "no cut term" in the extreme class
+    assert t[3, 17] == 100.0 and t[4, 17] == 0.0 and t[4, 7] == 0.0  # rt^2; 0 marks "no cut term" in the extreme class
     e = 0.9993
-    assert t[3, 17] == e / (1 + math.sqrt(1 - e * e))  # eps slot
+    assert t[3, 20] == e / (1 + math.sqrt(1 - e * e))  # eps slot
 
 
 def test_pack_constants():
-    """Per-lens constants: recomputed here from their definitions."""
+    """Per-lens constants (lh_pack.h): recomputed here from their definitions."""
     L = li.lens(li.DPIE, 1.5, -2.0, 0.6, 0.3, 0.25, 40.0, 3.0)
     t, _ = lh.lh_pack_model(L)
     k = t[0]
-    eps = 1.0 / 3.0  # e-hat 0.6 <-> eps 1/3 (reading 8c-2)
+    eps = 1.0 / 3.0  # e-hat 0.6 <-> eps 1/3 (reading R2)
     o, p, m = 1 - eps ** 2, (1 + eps) ** 2, (1 - eps) ** 2
     T = 3.0 * 40.0 / (40.0 - 0.25)
-    se = 2 * math.sqrt(eps) / o  # sec. 5.2 divided by o: one uniform operand per instruction
-    G = T / se
-    want = [1.5, -2.0, math.cos(0.3), math.sin(0.3), 1 / p, 1 / m, 0.25 ** 2, 40.0 ** 2, o, se, p / o * 0.25,
-            p / o * 40.0, m / o * 0.25, m / o * 40.0, math.cos(0.3) * G, math.sin(0.3) * G, T]
-    assert np.allclose(k[:17], want, rtol=4e-16, atol=0)
-    assert np.allclose(k[18:], [2 * o * 0.25, 2 * o * 40.0, 2 * (1 + eps ** 2) * 0.0625, 2 * (1 + eps ** 2) * 1600,
-                                -4 * eps * math.cos(0.6) * T, -2 * eps * math.sin(0.6) * T], rtol=1e-15)
-    # circular lens: the 2 sqrt(eps) -> 0 limit is taken with a tiny stand-in, G se = T o stays exact
+    sg = 2 * math.sqrt(eps)
+    kk = o / sg  # the lens frame is carried scaled by k = o / (2 sqrt eps)
+    G, TF = T * kk, T * kk * p / sg ** 2
+    want = [1.5, -2.0, math.cos(0.3), math.sin(0.3), kk * kk / p, kk * kk / m, kk * kk * 0.25 ** 2, kk * kk * 40.0 ** 2,
+            p / sg * 0.25, p / sg * 40.0, m / sg * 0.25, m / sg * 40.0, math.cos(0.3) * G, math.sin(0.3) * G, G, TF,
+            0.25 ** 2, 40.0 ** 2, -4 * eps * math.cos(0.6) * TF, -2 * eps * math.sin(0.6) * TF, eps, o, sg, T]
+    assert np.allclose(k, want, rtol=1e-15, atol=0)
+    # circular lens: 2 sqrt(eps) is never below 2^-64 (the scaled frame then takes the eps -> 0 limit exactly)
     k0 = lh.lh_pack_model(li.lens(li.DPIE, 0.0, 0.0, 0.0, 0.0, 0.25, 40.0, 3.0))[0][0]
-    assert k0[9] == 2.0 ** -500 and k0[14] * k0[9] == T and k0[15] == 0.0 and k0[22] == 0.0 and k0[23] == 0.0
+    assert k0[22] == 2.0 ** -64 and k0[14] == T * 2.0 ** 64 and k0[13] == 0.0 and k0[18] == 0.0 and k0[19] == 0.0
+    assert k0[4] == 2.0 ** 128 and k0[8] == 0.25 * 2.0 ** 64
+    # SIS: only the centre and b0 are used
+    ks = lh.lh_pack_model(li.lens(li.SIS, 2.0, 3.0, 0.0, 0.0, 0.0, 0.0, 0.7))[0][0]
+    assert ks[0] == 2.0 and ks[1] == 3.0 and ks[14] == 0.7
 
 
 @pytest.mark.parametrize("field,value,ok", [
