@@ -2,7 +2,7 @@
 """bench.py -- pixel-lens FP64 gradient+Hessian evaluations per second on B200.
 
 A "step" is one pass of the whole hot path (rows a1-a5: pack the lens
-list, stage the table, superpose first and second derivatives over all lenses at every
+list, hand the records to the launches, superpose first and second derivatives over all lenses at every
 pixel, fused kappa/gamma/mu epilogue, stores) over BASELINE.json config 3:
 4096 x 4096 pixels x 1000 dPIE potentials, outputs ax ay kappa gamma1 gamma2 mu, the
 Hessian never written.  One process per GPU; at N > 1 every rank evaluates its own lens
@@ -36,18 +36,22 @@ import lens_inputs as li  # noqa: E402
 METRIC = "pixel-lens FP64 gradient+Hessian evals/sec"
 UNIT = "evals/s"
 
-# Executed FP64 flops per (pixel, lens) evaluation of the timed kernel variant (gradient +
-# Hessian, dPIE), from the ncu counters (2*dfma + dadd + dmul thread-instructions) / evals:
-# profiles/r01_ncu_cfg3.md.  DESIGN.md sec. 7 derives the same figure from the SASS.
-FLOPS_PER_EVAL = {"grad+hess": 0.0, "grad": 0.0, "hess": 0.0}
-# SURVEY.md sec. 8(d) canonical count for the cheapest exact formulation it knew (context)
+# Executed FP64 flops per (pixel, lens) dPIE evaluation of each kernel variant (2*DFMA + DMUL + DADD
+# thread-instructions / evaluations).  grad+hess: ncu counters, profiles/r01_cfg3_ncu.md (84.0 FP64
+# instructions, 123.0 flop); grad / hess: the same count read from the SASS inner loop (59.5 and 47
+# instructions).  DESIGN.md sec. 7.  This is what the hardware did -- `roofline.achieved` never claims more.
+FLOPS_PER_EVAL = {"grad+hess": 123.0, "grad": 87.5, "hess": 70.0}
+FP64_INSTR_PER_EVAL = {"grad+hess": 84.0, "grad": 59.5, "hess": 47.0}
+# SURVEY.md sec. 8(d) canonical count for the cheapest exact formulation it knew (context: this kernel's
+# formulation is cheaper, so evals/s x canonical flops can exceed the FLOP/s peak and is NOT a roofline fraction)
 CANONICAL_FLOPS_PER_EVAL = {"grad+hess": 278.0, "grad": 205.0, "hess": 105.0}
 # FP64 CUDA-core peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x SM clock (B200_PROFILING.md:
 # 148 SMs, clocks.max.sm 1965 MHz).  The live DFMA probe (lh_fp64_peak_probe) is the
 # measured counterpart and is what `roofline.peak` reports.
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# dram bytes (read+write) per launch of the timed kernel from `ncu --set full` (profiles/); None until captured
-NCU_TRAFFIC_BYTES = {3: None}
+# dram bytes (read+write) per launch of the timed kernel from `ncu --set full` (profiles/r01_cfg3_ncu.md:
+# a middle lens chunk of cfg 3 reads and writes the five carried accumulators)
+NCU_TRAFFIC_BYTES = {3: 1.290e9}
 
 
 def parse():
@@ -163,8 +167,8 @@ def workload_config(cfg, args):
                         + (f" x {cfg.nmodel} models" if cfg.nmodel > 1 else ""),
             "outputs": list(cfg.outputs), "evals_per_step_per_gpu": cfg.evals,
             "l2": "output planes (%d MiB/step) exceed the 126 MB L2 and a 256 MiB buffer is rewritten between "
-                  "timed steps; the lens table (%d KiB) is cache-resident by design"
-                  % (len(cfg.outputs) * cfg.nmodel * g.npix * 8 >> 20, cfg.nmodel * cfg.nlens * 224 >> 10),
+                  "timed steps; the lens records (%d KiB) travel in the kernel parameters"
+                  % (len(cfg.outputs) * cfg.nmodel * g.npix * 8 >> 20, cfg.nmodel * cfg.nlens * 192 >> 10),
             "parallelism": f"independent lens models per GPU x{args.gpus}, no collective"}
 
 
@@ -249,7 +253,7 @@ def run_ours(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t.item())
         e2e = {"value": world * cfg.evals * k_e2e / dt, "unit": UNIT,
-               "h2d_bytes_per_step": int(cfg.nmodel * cfg.nlens * 224 + cfg.nmodel * 16),
+               "h2d_bytes_per_step": int(cfg.nmodel * cfg.nlens * 192 + cfg.nmodel * 8),
                "d2h_bytes_per_step": int(len(cfg.outputs) * cfg.nmodel * g.npix * 8),
                "ms_per_step": 1e3 * dt / k_e2e, "steps": k_e2e,
                "note": "lh_grid_eval_host: host lens list in, pinned host planes out, packing + copies + sync timed"}
@@ -265,20 +269,29 @@ def run_ours(args):
     peak_flops, _ = lh.lh_fp64_peak_probe(1 << 15)
     mode = "grad+hess" if (set(cfg.outputs) & {"ax", "ay"}) and (set(cfg.outputs) - {"ax", "ay"}) else (
         "grad" if set(cfg.outputs) <= {"ax", "ay"} else "hess")
-    fpe = FLOPS_PER_EVAL[mode] or CANONICAL_FLOPS_PER_EVAL[mode]
-    kernel_s = float(np.mean(step_ms)) * 1e-3
-    achieved = fpe * cfg.evals / kernel_s / 1e12
+    fpe = FLOPS_PER_EVAL[mode]
+    step_s = float(np.mean(step_ms)) * 1e-3
+    per_step = launches / args.steps
+    launch_s = step_s / per_step          # average duration of one superpose_kernel launch (CUDA events)
+    launch_evals = cfg.evals / per_step   # units one launch processes
+    achieved = fpe * launch_evals / launch_s / 1e12
+    instr_rate = FP64_INSTR_PER_EVAL[mode] * launch_evals / launch_s  # FP64 thread-instructions / s
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_flops / 1e12, "unit": "TFLOP/s",
                 "frac": achieved / (peak_flops / 1e12), "traffic": NCU_TRAFFIC_BYTES.get(args.config),
                 "peak_source": "measured live: lh_fp64_peak_probe (DFMA chains, all SMs); nominal "
-                               f"{NOMINAL_FP64_TFLOPS:.1f} TFLOP/s = 148 SM x 64 lanes x 2 x 1.965 GHz",
+                               f"{NOMINAL_FP64_TFLOPS:.1f} TFLOP/s = 148 SM x 64 lanes x 2 x 1.965 GHz "
+                               "(MEASURED_PEAKS.json has no FP64 entry)",
                 "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
-                "flops_per_eval": fpe, "flops_per_eval_source": "ncu-counted executed FP64 flops" if
-                FLOPS_PER_EVAL[mode] else "SURVEY 8(d) canonical count (no ncu count yet)",
+                "flops_per_eval": fpe, "flops_per_eval_source": "executed FP64 flops (ncu / SASS), dPIE, " + mode,
+                "fp64_issue_frac": instr_rate / (148 * 64 * 1.965e9),
+                "fp64_issue_note": "FP64 thread-instructions/s over 148 x 64 lanes x 1.965 GHz; only "
+                                   f"{100 * (fpe / FP64_INSTR_PER_EVAL[mode] - 1):.0f} % of them are FMAs, and every non-FP64 "
+                                   "instruction costs a dispatch cycle of the same port (DESIGN.md sec. 7)",
                 "canonical_flops_per_eval": CANONICAL_FLOPS_PER_EVAL[mode],
-                "achieved_canonical": CANONICAL_FLOPS_PER_EVAL[mode] * cfg.evals / kernel_s / 1e12,
-                "kernel_ms": kernel_s * 1e3, "kernel": "lh::superpose_kernel<%s>" % mode,
-                "store_gbs": len(cfg.outputs) * cfg.nmodel * g.npix * 8 / kernel_s / 1e9}
+                "achieved_canonical": CANONICAL_FLOPS_PER_EVAL[mode] * cfg.evals / step_s / 1e12,
+                "kernel": "lh::superpose_kernel<%s>" % mode, "launches_per_step": per_step,
+                "kernel_ms": launch_s * 1e3, "units_per_launch": launch_evals,
+                "store_gbs": len(cfg.outputs) * cfg.nmodel * g.npix * 8 / step_s / 1e9}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",

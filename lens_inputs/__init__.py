@@ -192,3 +192,27 @@ def random_points(seed: int, grid: Grid, n: int):
     flat = rng.choice(grid.npix, size=min(n, grid.npix), replace=False)
     flat.sort()
     return (flat % grid.nx).astype(np.int64), (flat // grid.nx).astype(np.int64)
+
+
+# ---------------------------------------------------------------- sharding
+def row_slab(grid: Grid, rank: int, world: int):
+    """Contiguous row slab of `grid` owned by `rank` of `world` (pixels are independent):
+    returns (sub-grid, first row j0).  Rows are split as evenly as possible, earlier ranks take the extra
+    rows; a rank may own zero rows (sub-grid ny = 0) when world > grid.ny.  The sub-grid is the SAME
+    lattice: y0 + j0*dx is computed once here, and the kernel's y0_slab + j*dx can differ from the full
+    map's y0 + (j0+j)*dx by one rounding unless dx and y0 are dyadic (they are for every BASELINE config)."""
+    if not (0 <= rank < world):
+        raise ValueError("rank outside [0, world)")
+    base, extra = divmod(grid.ny, world)
+    rows = base + (1 if rank < extra else 0)
+    j0 = rank * base + min(rank, extra)
+    return Grid(x0=grid.x0, y0=grid.y0 + j0 * grid.dx, dx=grid.dx, nx=grid.nx, ny=rows), j0
+
+
+def model_slab(nmodel: int, rank: int, world: int):
+    """Models [m0, m1) of a batch owned by `rank` (batch path shards by model, no exchange)."""
+    if not (0 <= rank < world):
+        raise ValueError("rank outside [0, world)")
+    base, extra = divmod(nmodel, world)
+    m0 = rank * base + min(rank, extra)
+    return m0, m0 + base + (1 if rank < extra else 0)

@@ -34,6 +34,12 @@ namespace lh {
 #ifndef LH_MINB
 #define LH_MINB 4  // CTAs per SM the register allocation is held to (__launch_bounds__)
 #endif
+#ifndef LH_MINB_GRAD
+#define LH_MINB_GRAD 6  // gradient-only variant
+#endif
+#ifndef LH_MINB_HESS
+#define LH_MINB_HESS 5  // Hessian-only variant
+#endif
 constexpr int PX = LH_PX;
 constexpr int TILE_W = 32 * PX;    // one warp spans 32*PX pixels of a row
 constexpr int TILE_H = LH_WARPS;
@@ -209,8 +215,16 @@ __device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc
 // only while it reads at most two distinct vector registers; an FMA with three costs 3
 // (profiles/r01_fp64_operand_probe.md).  A record staged in shared memory would land in
 // vector registers and make almost every FMA of the lens algebra a 3-register one.
+//
+// ptxas only moves the record fields to the uniform datapath (LDCU) when the vector register
+// budget is tight; with room to spare it loads them into vector registers (LDC) and the FMAs
+// become 3-register ones again.  The CTAs-per-SM figure of __launch_bounds__ is therefore
+// chosen per variant so that the budget IS tight (tests/test_sass_cpu.py checks the outcome).
+template <bool GRAD, bool HESS>
+constexpr int min_blocks() { return (GRAD && HESS) ? LH_MINB : (GRAD ? LH_MINB_GRAD : LH_MINB_HESS); }
+
 template <bool GRAD, bool HESS, bool EXTREME>
-__global__ void __launch_bounds__(THREADS, EXTREME ? 1 : LH_MINB) superpose_kernel(const __grid_constant__ LaunchParams P) {
+__global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>()) superpose_kernel(const __grid_constant__ LaunchParams P) {
     __shared__ SmemTables tb;
 
     // reduction tables of atan / atanh: global (L2-resident, 18 KB) -> shared, once per CTA

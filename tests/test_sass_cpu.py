@@ -1,0 +1,73 @@
+"""Static checks on the compiled kernels (cuobjdump, no GPU): the properties DESIGN.md sec. 7 relies on.
+
+1. The lens records are read through the uniform datapath (LDCU c[0x0][UR..]) in every fast
+   kernel variant -- never through vector-indexed LDC, which would put the constants in vector
+   registers and make the lens algebra's FMAs three-register (3-cycle) ones.
+2. No local-memory spills, no libdevice slow paths (calls) in the fast variants.
+"""
+import re
+import shutil
+import subprocess
+
+import pytest
+
+import paper_2004_06352_b200 as lh
+
+CUOBJDUMP = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+
+
+@pytest.fixture(scope="module")
+def sass():
+    try:
+        out = subprocess.run([CUOBJDUMP, "-sass", lh.library_path()], capture_output=True, text=True, check=True).stdout
+    except (OSError, subprocess.CalledProcessError) as e:  # pragma: no cover
+        pytest.skip(f"cuobjdump unavailable: {e}")
+    funcs, name = {}, None
+    for line in out.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            name = m.group(1)
+            funcs[name] = []
+        elif name:
+            funcs[name].append(line)
+    return funcs
+
+
+FAST = ["ILb1ELb1ELb0", "ILb1ELb0ELb0", "ILb0ELb1ELb0"]  # <GRAD, HESS, EXTREME = false>
+
+
+@pytest.mark.parametrize("variant", FAST)
+def test_lens_records_come_through_uniform_registers(sass, variant):
+    name = next(n for n in sass if "superpose_kernel" in n and variant in n)
+    body = "\n".join(sass[name])
+    vector_indexed = re.findall(r"LDC(?:\.\d+)? R\d+, c\[0x0\]\[R\d+", body)
+    uniform_indexed = re.findall(r"LDCU(?:\.\d+)? UR\d+, c\[0x0\]\[UR\d+", body)
+    assert not vector_indexed, f"{name}: {len(vector_indexed)} vector-indexed parameter loads (lens fields in vector registers)"
+    assert len(uniform_indexed) >= 10
+    assert re.search(r"D(FMA|MUL|ADD) R\d+, [^;]*UR\d+", body), "no FP64 instruction takes a uniform operand"
+
+
+@pytest.mark.parametrize("variant", FAST)
+def test_no_spills_and_no_calls_in_fast_variants(sass, variant):
+    name = next(n for n in sass if "superpose_kernel" in n and variant in n)
+    body = "\n".join(sass[name])
+    assert not re.search(r"\b(STL|LDL)\b", body), "local-memory traffic (register spill)"
+    # the only calls allowed are the IEEE-division slow paths of the per-pixel epilogue (mu = 1/det),
+    # which sit after the last lens loop
+    last_backedge, calls = -1, []
+    for line in sass[name]:
+        m = re.search(r"/\*([0-9a-f]{4,})\*/\s+(?:@!?U?P\d\s+)?(BRA(?:\.U)?|CALL\S*)\s+(?:!?U?P\d,\s+)?0x([0-9a-f]+)", line)
+        if not m:
+            continue
+        at, op, to = int(m.group(1), 16), m.group(2), int(m.group(3), 16)
+        if op.startswith("BRA") and to < at:
+            last_backedge = max(last_backedge, at)
+        if op.startswith("CALL"):
+            calls.append(at)
+    assert last_backedge > 0
+    assert all(c > last_backedge for c in calls), "a slow-path call inside a lens loop of a fast variant"
+
+
+def test_extreme_variants_exist_and_use_libdevice_paths(sass):
+    names = [n for n in sass if "superpose_kernel" in n and n.endswith("ELb1EEEvNS_12LaunchParamsE")]
+    assert len(names) == 3
