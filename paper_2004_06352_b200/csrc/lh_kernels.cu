@@ -74,13 +74,12 @@ __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Ac
     rsqrt_sqrt(L.rt2 + rho2, wt, iwt);
     const double Pc = wc + L.ac, Pt = wt + L.at;
     Reduced ra, rh;
-    double nx = 0.0, ny = 0.0, Dc = 1.0, Dt = 1.0, i1, i2, i3, i4;
+    double Dc = 1.0, Dt = 1.0, i1, i2, i3, i4;
     if (GRAD) {
+        // P^_t > P^_c and Q^_t > Q^_c (rcut > rcore): the arguments carry the signs of x' and y'
         const double Qc = wc + L.bc, Qt = wt + L.bt;
-        nx = xp * (Pt - Pc);
-        ny = yp * (Qt - Qc);
-        ra = atan_reduce(nx, fma(xp, xp, Pc * Pt), tb.at);
-        rh = atanh_reduce(ny, fma(-yp, yp, Qc * Qt), tb.ah);
+        ra = atan_reduce(fabs(xp) * (Pt - Pc), fma(xp, xp, Pc * Pt), tb.at);
+        rh = atanh_reduce(fabs(yp) * (Qt - Qc), fma(-yp, yp, Qc * Qt), tb.ah);
     }
     if (HESS) {
         Dc = fma(Pc, Pc, xx);
@@ -93,8 +92,8 @@ __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Ac
     else
         rcp2(Dc, Dt, i3, i4);
     if (GRAD) {
-        const double at = atan_finish(ra, i1, nx);
-        const double ah = atanh_finish(rh, i2, ny);
+        const double at = atan_finish(ra, i1, xp);
+        const double ah = atanh_finish(rh, i2, yp);
         a.ax = fma(L.cG, at, fma(-L.sG, ah, a.ax));
         a.ay = fma(L.sG, at, fma(L.cG, ah, a.ay));
     }
@@ -120,8 +119,8 @@ __device__ __forceinline__ void nsie_term(const LensK &L, double X, double Y, Ac
     rsqrt_sqrt(L.rc2 + rho2, wc, iwc);
     const double Pc = wc + L.ac;
     if (GRAD) {
-        const Reduced ra = atan_reduce(xp, Pc, tb.at);
-        const Reduced rh = atanh_reduce(yp, wc + L.bc, tb.ah);
+        const Reduced ra = atan_reduce(fabs(xp), Pc, tb.at);
+        const Reduced rh = atanh_reduce(fabs(yp), wc + L.bc, tb.ah);
         double i1, i2;
         rcp2(ra.den, rh.den, i1, i2);
         const double at = atan_finish(ra, i1, xp);

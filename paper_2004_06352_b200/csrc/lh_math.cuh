@@ -128,9 +128,7 @@ LH_HD void rsqrt_sqrt(double v, double &w, double &iw) {
     w = fma(t, h, t);
 }
 
-// |x| and copysign as integer operations on the high word (1 dispatch cycle, not 2)
-LH_HD double fabs_i(double x) { return mk64(hi32(x) & 0x7fffffff, lo32(x)); }
-// mag >= 0: one LOP3
+// copysign as ONE integer operation on the high word (1 dispatch cycle, not 2); mag >= 0
 LH_HD double copysign_pos_i(double mag, double sgn) { return mk64(hi32(mag) | (hi32(sgn) & (int)0x80000000), lo32(mag)); }
 
 // Table index of a positive quotient q (approximate is enough): exponent and top 6 mantissa
@@ -150,8 +148,7 @@ LH_HD unsigned quot_index(double q, int oct_min, int n) {
 // k = 0..63, is t_c = 2^-(o+1) (2 - k/64) ... i.e. the exponent/6-bit-mantissa code of t
 // subtracted from that of 1.0.  t above 1 (rounding) maps to entry 0, t below the table to the last.
 LH_HD unsigned quot_index_down(double t, int n) {
-    const int hr = hi32(t) + 0x2000;
-    const int j = (1023 << 6) - (hr >> 14);
+    const int j = ((1023 << 20) + 0x2000 - hi32(t)) >> 14;  // round((code(1.0) - code(t)) / 2^14)
 #ifdef __CUDA_ARCH__
     return min((unsigned)max(j, 0), (unsigned)(n - 1));
 #else
@@ -159,56 +156,55 @@ LH_HD unsigned quot_index_down(double t, int n) {
 #endif
 }
 
-// ---- atan(n/d), d > 0, any finite n -----------------------------------------------------------
+// ---- atan(n/d), d > 0 -------------------------------------------------------------------------
 // Split in two so that the caller can share the reciprocal of the reduced denominator with
-// other reciprocals (rcp2 / rcp4):
-//   atan_reduce: an = |n|, pick c, return num = an - c d and den = d + c an (> 0)   3 FP64 + 1 MUFU
-//   atan_finish: z = num/den given 1/den, atan c + z (1 - z^2/3 + z^4/5), sign of n 5 FP64
+// other reciprocals (rcp2 / rcp4), and fed with an = |n| so that the caller can fold the
+// absolute value into the instruction that produces n (|x| operand modifiers are free):
+//   atan_reduce: pick c, return num = an - c d and den = d + c an (> 0)             3 FP64 + 1 MUFU
+//   atan_finish: z = num/den given 1/den, atan c + z (1 - z^2/3 + z^4/5), sign of `sgn`  5 FP64
 struct Reduced {
     double num, den, base;
 };
-LH_HD Reduced atan_reduce(double n, double d, const double2 *__restrict__ tab) {
-    const double an = fabs_i(n);
+LH_HD Reduced atan_reduce(double an, double d, const double2 *__restrict__ tab) {
     const double q0 = an * rcp_seed(d);  // |n|/d to 1e-6
     const double2 ca = tab[quot_index(q0, ATAN_OCT_MIN, ATAN_N)];
     return Reduced{fma(-ca.x, d, an), fma(ca.x, an, d), ca.y};
 }
-LH_HD double atan_finish(const Reduced &r, double iden, double n) {
+LH_HD double atan_finish(const Reduced &r, double iden, double sgn) {
     const double z = r.num * iden;  // |z| <= 2^-8
     const double z2 = z * z;
     const double p = fma(z2, fma(z2, 0.2, -1.0 / 3.0), 1.0);
-    return copysign_pos_i(fma(z, p, r.base), n);
+    return copysign_pos_i(fma(z, p, r.base), sgn);
 }
 
-// ---- atanh(n/d), 0 <= |n| < d with 1 - |n|/d > 2^-16 -----------------------------------------
-// u = |n|/d; the bin is chosen on t = 1 - u = (d-|n|)/d, whose exponent follows the singularity
+// ---- atanh(n/d), 0 <= an = |n| < d with 1 - an/d > 2^-16 --------------------------------------
+// u = an/d; the bin is chosen on t = 1 - u = (d-an)/d, whose exponent follows the singularity
 // of atanh at u = 1: bins are t_c = 2^-e (1 + k/64), c' = 1 - t_c, so that the reduced argument
-//   s = (|n| - c' d)/(d - c' |n|) = (u - c')/(1 - c' u)
+//   s = (an - c' d)/(d - c' an) = (u - c')/(1 - c' u)
 // stays below 2^-7.5 everywhere (|u - c'| <= t/128 and 1 - c'u >= 1 - u^2 ~ 2t near u = 1).
-// Both FMAs see the exact n and d.  The host packer (lh_pack.cpp) routes every lens whose
+// Both FMAs see the exact an and d.  The host packer (lh_pack.cpp) routes every lens whose
 // ellipticity could push u past the table into the CLS_EXTREME class, which does not come
 // through here; the index is clamped all the same.
 //   atanh_reduce  4 FP64 + 1 MUFU      atanh_finish  5 FP64
-LH_HD Reduced atanh_reduce(double n, double d, const double2 *__restrict__ tab) {
-    const double an = fabs_i(n);
+LH_HD Reduced atanh_reduce(double an, double d, const double2 *__restrict__ tab) {
     const double t0 = (d - an) * rcp_seed(d);  // 1 - u to 1e-6 relative
     const double2 ca = tab[quot_index_down(t0, LN_N)];
     return Reduced{fma(-ca.x, d, an), fma(-ca.x, an, d), ca.y};
 }
-LH_HD double atanh_finish(const Reduced &r, double iden, double n) {
+LH_HD double atanh_finish(const Reduced &r, double iden, double sgn) {
     const double s = r.num * iden;
     const double s2 = s * s;
     const double p = fma(s2, fma(s2, 0.2, 1.0 / 3.0), 1.0);
-    return copysign_pos_i(fma(s, p, r.base), n);
+    return copysign_pos_i(fma(s, p, r.base), sgn);
 }
 
-// Stand-alone forms (one reciprocal each)
+// Stand-alone forms (one reciprocal each), any sign of n
 LH_HD double atan_nd(double n, double d, const double2 *__restrict__ tab) {
-    const Reduced r = atan_reduce(n, d, tab);
+    const Reduced r = atan_reduce(fabs(n), d, tab);
     return atan_finish(r, rcp(r.den), n);
 }
 LH_HD double atanh_nd(double n, double d, const double2 *__restrict__ tab) {
-    const Reduced r = atanh_reduce(n, d, tab);
+    const Reduced r = atanh_reduce(fabs(n), d, tab);
     return atanh_finish(r, rcp(r.den), n);
 }
 
