@@ -26,13 +26,13 @@
 namespace lh {
 
 #ifndef LH_PX
-#define LH_PX 2  // pixels per thread (adjacent in x -> one double2 store per plane)
+#define LH_PX 4  // pixels per thread (adjacent in x -> double2 stores; per-lens uniform loads amortised over 4)
 #endif
 #ifndef LH_WARPS
-#define LH_WARPS 4  // warps per CTA, one grid row each
+#define LH_WARPS 2  // warps per CTA, one grid row each
 #endif
 #ifndef LH_MINB
-#define LH_MINB 4  // CTAs per SM the register allocation is held to (__launch_bounds__)
+#define LH_MINB 5  // CTAs per SM the register allocation is held to (__launch_bounds__), gradient + Hessian variant
 #endif
 #ifndef LH_MINB_GRAD
 #define LH_MINB_GRAD 6  // gradient-only variant
