@@ -118,15 +118,17 @@ def test_cfg4_full_size_batch_sampled():
 @pytest.mark.parametrize("nx,ny", [(1, 1), (1, 9), (9, 1), (63, 3), (64, 4), (65, 5), (67, 7), (129, 2), (200, 13)])
 def test_ragged_grids(nx, ny):
     c = li.config(2)
-    L = c.lenses[:130]  # 3 tiles of 64 minus a tail; dPIE + NSIE + SIS
+    L = c.lenses[:130]  # dPIE + NSIE + SIS in one launch
     g = li.Grid(x0=-20.3, y0=11.7, dx=0.37, nx=nx, ny=ny)
     ref = ref_grid(L, g, li.ALL_PLANES)
     got = run_gpu(L, g, li.ALL_PLANES)
     check_planes(got, ref, f"ragged {nx}x{ny}")
 
 
-@pytest.mark.parametrize("nlens", [0, 1, 63, 64, 65, 128, 129])
-def test_lens_counts_around_tile_size(nlens):
+@pytest.mark.parametrize("nlens", [0, 1, 63, 159, 160, 161, 320, 321, 481])
+def test_lens_counts_around_launch_capacity(nlens):
+    """A launch carries at most 160 records in its kernel parameters (lh_kernels.h); more lenses are evaluated by
+    consecutive launches that hand the accumulators on through the carry buffer."""
     c = li.config(3)
     L = c.lenses[:nlens]
     g = li.Grid(x0=-30.0, y0=-30.0, dx=0.9, nx=70, ny=9)
@@ -136,6 +138,57 @@ def test_lens_counts_around_tile_size(nlens):
     if nlens == 0:
         for n in got:
             assert np.all(got[n] == (1.0 if n == "mu" else 0.0))
+
+
+def test_many_small_models_share_launches():
+    """Models with few lenses share one launch (blockIdx.y); 50 x 7 records need three launches of <= 22 models."""
+    c = li.config(2)
+    rng = np.random.default_rng(5)
+    nmodel, nlens = 50, 7
+    L = c.lenses[rng.integers(0, len(c.lenses), nmodel * nlens)]  # dPIE / NSIE / SIS mix differs per model
+    g = li.Grid(x0=-40.0, y0=-25.0, dx=0.77, nx=131, ny=5)
+    n0 = lh.lh_launch_count()
+    got = run_gpu(L, g, li.ALL_PLANES, nmodel=nmodel, nlens=nlens)
+    assert lh.lh_launch_count() - n0 == 3
+    for m in range(nmodel):
+        ref = ref_grid(L[m * nlens:(m + 1) * nlens], g, li.ALL_PLANES)
+        check_planes({n: got[n][m] for n in got}, ref, f"small model {m}")
+
+
+def test_batch_of_empty_models():
+    g = li.Grid(x0=0.0, y0=0.0, dx=1.0, nx=33, ny=3)
+    got = run_gpu(li.make_lenses(0), g, li.ALL_PLANES, nmodel=200, nlens=0)
+    for n in got:
+        assert got[n].shape == (200, 3, 33) and np.all(got[n] == (1.0 if n == "mu" else 0.0))
+
+
+def test_chunked_model_with_every_class():
+    """> 160 lenses with dPIE, NSIE, SIS and extreme-ellipticity lenses: class boundaries fall inside and on
+    the edges of the lens chunks; also as a batch of two such models (chunks run model by model)."""
+    c = li.config(2)
+    L = c.lenses[:330].copy()
+    L["ellipticity"][[5, 170, 171, 329]] = 0.9995  # CLS_EXTREME (sorted last by the packer)
+    g = li.Grid(x0=-60.0, y0=-60.0, dx=1.3, nx=93, ny=21)
+    rel = conditioned_rel(0.9995)
+    check_planes(run_gpu(L, g, li.ALL_PLANES), ref_grid(L, g, li.ALL_PLANES), "chunked, all classes", rel=rel)
+    L2 = np.concatenate([L, L[::-1]])
+    got = run_gpu(L2, g, ("ax", "kappa", "mu"), nmodel=2, nlens=330)
+    for m in range(2):
+        ref = ref_grid(L2[m * 330:(m + 1) * 330], g, ("ax", "kappa", "mu"))
+        check_planes({n: got[n][m] for n in got}, ref, f"chunked batch model {m}", rel=rel)
+
+
+def test_extreme_length_scales_stay_inside_the_shared_reciprocal_range():
+    """rcp4 takes the reciprocal of a product of four squared lengths (include/lh.h: lengths within ~1e+-35):
+    micro-arcsec and 1e12-arcsec units must still give oracle-grade results."""
+    for scale in (1e-9, 1e12):
+        L = li.make_lenses(2)
+        L[0] = (li.DPIE, 0, 0.3 * scale, -0.2 * scale, 0.4, 0.7, 0.08 * scale, 30.0 * scale, 1.7 * scale)
+        L[1] = (li.DPIE, 0, -4.0 * scale, 2.0 * scale, 0.0, 0.0, 0.5 * scale, 9.0 * scale, 0.6 * scale)
+        g = li.Grid(x0=-15.0 * scale, y0=-15.0 * scale, dx=0.61 * scale, nx=49, ny=49)
+        got = run_gpu(L, g, li.ALL_PLANES)
+        check_planes(got, ref_grid(L, g, li.ALL_PLANES), f"scale {scale}")
+        assert all(np.isfinite(v).all() for v in got.values())
 
 
 def test_mixed_types_any_order():
