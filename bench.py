@@ -37,11 +37,11 @@ METRIC = "pixel-lens FP64 gradient+Hessian evals/sec"
 UNIT = "evals/s"
 
 # Executed FP64 flops per (pixel, lens) dPIE evaluation of each kernel variant (2*DFMA + DMUL + DADD
-# thread-instructions / evaluations).  grad+hess: ncu counters, profiles/r01_cfg3_ncu.md (84.0 FP64
-# instructions, 123.0 flop); grad / hess: the same count read from the SASS inner loop (59.5 and 47
+# thread-instructions / evaluations).  grad+hess: ncu counters, profiles/r01_cfg3_ncu.md (83.0 FP64
+# instructions, 122.0 flop); grad / hess: the same count read from the SASS inner loop (58.75 and 46
 # instructions).  DESIGN.md sec. 7.  This is what the hardware did -- `roofline.achieved` never claims more.
-FLOPS_PER_EVAL = {"grad+hess": 123.0, "grad": 87.5, "hess": 70.0}
-FP64_INSTR_PER_EVAL = {"grad+hess": 84.0, "grad": 59.5, "hess": 47.0}
+FLOPS_PER_EVAL = {"grad+hess": 122.0, "grad": 86.75, "hess": 69.0}
+FP64_INSTR_PER_EVAL = {"grad+hess": 83.0, "grad": 58.75, "hess": 46.0}
 # SURVEY.md sec. 8(d) canonical count for the cheapest exact formulation it knew (context: this kernel's
 # formulation is cheaper, so evals/s x canonical flops can exceed the FLOP/s peak and is NOT a roofline fraction)
 CANONICAL_FLOPS_PER_EVAL = {"grad+hess": 278.0, "grad": 205.0, "hess": 105.0}
