@@ -62,24 +62,27 @@ using SmemTables = MathTables;  // the atan / atanh reduction tables, staged per
 //   a11 - a22 += TF [ K (f^_c rc^2 - f^_t rt^2) - (dx^2 - dy^2)(f^_c - f^_t) ],  K  = -4 eps cos 2theta
 //   a12       += TF [ K'(f^_c rc^2 - f^_t rt^2) -  dx dy       (f^_c - f^_t) ],  K' = -2 eps sin 2theta
 // The four reciprocals (reduced atan / atanh denominators, D^_c, D^_t) come from ONE seed (rcp4).
+// RULE: no FP64 instruction may take TWO lens fields.  One of them would have to be copied into a
+// vector register, and ptxas then gives up the uniform datapath for the whole record (vector LDC,
+// 3-register FMAs everywhere) -- measured, and guarded by tests/test_sass_cpu.py.
 template <bool GRAD, bool HESS>
 __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Acc &a, const SmemTables &tb) {
     const double dx = X - L.xc, dy = Y - L.yc;
     const double xp = fma(L.c, dx, L.s * dy);
     const double yp = fma(-L.s, dx, L.c * dy);
     const double xx = xp * xp, yy = yp * yp;
-    const double rho2 = fma(L.ip, xx, L.im * yy);
+    const double vc = fma(L.ip, xx, L.im * yy) + L.rc2;  // k^2 (rc^2 + rho^2)
     double wc, iwc, wt, iwt;
-    rsqrt_sqrt(L.rc2 + rho2, wc, iwc);
-    rsqrt_sqrt(L.rt2 + rho2, wt, iwt);
+    rsqrt_sqrt(vc, wc, iwc);
+    rsqrt_sqrt(vc + L.dr2, wt, iwt);  // k^2 (rt^2 + rho^2)
     const double Pc = wc + L.ac, Pt = wt + L.at;
     Reduced ra, rh;
     double Dc = 1.0, Dt = 1.0, i1, i2, i3, i4;
     if (GRAD) {
         // P^_t > P^_c and Q^_t > Q^_c (rcut > rcore): the arguments carry the signs of x' and y'
         const double Qc = wc + L.bc, Qt = wt + L.bt;
-        ra = atan_reduce(fabs(xp) * (Pt - Pc), fma(xp, xp, Pc * Pt), tb.at);
-        rh = atanh_reduce(fabs(yp) * (Qt - Qc), fma(-yp, yp, Qc * Qt), tb.ah);
+        ra = atan_reduce(fabs(xp) * (Pt - Pc), fma(Pc, Pt, xx), tb.at);
+        rh = atanh_reduce(fabs(yp) * (Qt - Qc), fma(Qc, Qt, -yy), tb.ah);
     }
     if (HESS) {
         Dc = fma(Pc, Pc, xx);

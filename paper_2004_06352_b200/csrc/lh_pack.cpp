@@ -81,8 +81,8 @@ static void fill(const lh_lens &L, int cls, LensK &K) {
     K.r2t = rt * rt;
     K.KTF = -4.0 * eps * c2 * K.TF;
     K.K2TF = -2.0 * eps * s2 * K.TF;
+    K.dr2 = k * k * (rt * rt - rc * rc);
     K.eps = eps;
-    K.o = o;
     K.sg = sg;
     K.T = T;
 }

@@ -42,7 +42,7 @@ struct alignas(16) LensK {
     double G, TF;       // 14  G = T k (also the weight of 1/w^_c - 1/w^_t; SIS: b0);  TF = T k p / sg^2 (weight of f^_r)
     double r2c, r2t;    // 16  rcore^2, rcut^2 (unscaled)
     double KTF, K2TF;   // 18  -4 eps cos(2 theta) TF, -2 eps sin(2 theta) TF
-    double eps, o;      // 20  diagnostic
+    double dr2, eps;    // 20  k^2 (rcut^2 - rcore^2) = rt2 - rc2;  eps (diagnostic)
     double sg, T;       // 22  diagnostic
 };
 static_assert(sizeof(LensK) == 24 * 8, "LensK is 24 doubles");

@@ -68,7 +68,7 @@ def test_pack_routes_extreme_ellipticity_to_its_own_class():
     assert list(t[:, 0]) == [0.0, 4.0, 3.0, 1.0, 2.0]
     assert t[3, 17] == 100.0 and t[4, 17] == 0.0 and t[4, 7] == 0.0  # rt^2; 0 marks "no cut term" in the extreme class
     e = 0.9993
-    assert t[3, 20] == e / (1 + math.sqrt(1 - e * e))  # eps slot
+    assert t[3, 21] == e / (1 + math.sqrt(1 - e * e))  # eps slot
 
 
 def test_pack_constants():
@@ -84,7 +84,8 @@ def test_pack_constants():
     G, TF = T * kk, T * kk * p / sg ** 2
     want = [1.5, -2.0, math.cos(0.3), math.sin(0.3), kk * kk / p, kk * kk / m, kk * kk * 0.25 ** 2, kk * kk * 40.0 ** 2,
             p / sg * 0.25, p / sg * 40.0, m / sg * 0.25, m / sg * 40.0, math.cos(0.3) * G, math.sin(0.3) * G, G, TF,
-            0.25 ** 2, 40.0 ** 2, -4 * eps * math.cos(0.6) * TF, -2 * eps * math.sin(0.6) * TF, eps, o, sg, T]
+            0.25 ** 2, 40.0 ** 2, -4 * eps * math.cos(0.6) * TF, -2 * eps * math.sin(0.6) * TF,
+            kk * kk * (40.0 ** 2 - 0.25 ** 2), eps, sg, T]
     assert np.allclose(k, want, rtol=1e-15, atol=0)
     # circular lens: 2 sqrt(eps) is never below 2^-64 (the scaled frame then takes the eps -> 0 limit exactly)
     k0 = lh.lh_pack_model(li.lens(li.DPIE, 0.0, 0.0, 0.0, 0.0, 0.25, 40.0, 3.0))[0][0]
