@@ -114,6 +114,17 @@ int lh_grid_eval(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_ou
 /* Batched form of lh_grid_eval (layout as lh_grid_gradient_batch). */
 int lh_grid_eval_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *o);
 
+/* Per-pixel MEAN and VARIANCE of the requested planes over the `nmodel` lens models of a batch -- the
+ * statistical-error maps of the Bayesian process: "In order to compute the map variances, full-resolution
+ * lensing maps have to be generated for each tested parameter-combination" (sec. 2.4; 10014 maps
+ * for Abell 2744).  No per-model map is materialised: every model's planes are reduced in
+ * registers and folded into the running statistics (Welford) by the kernel epilogue, one launch chain per model
+ * in model order.  mean->P / var->P are single [ny][nx] DEVICE planes; var may be NULL, and a variance plane
+ * needs its mean plane.  Variance is the POPULATION variance (1/nmodel) sum (P_m - mean)^2 (R21).
+ * mu is +-inf on critical lines, so its statistics are IEEE inf/NaN there.  Errors as lh_grid_gradient. */
+int lh_grid_stats_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *mean,
+                        const lh_outputs *var);
+
 /* Same as lh_grid_eval_batch with HOST output planes: the library allocates (and
  * caches) device planes, runs the same kernel, copies the requested planes back
  * and synchronises the stream before returning.  This is the end-to-end path a

@@ -139,3 +139,29 @@ def grid(lenses, x0: float, y0: float, dx: float, nx: int, ny: int, planes=PLANE
         with ThreadPoolExecutor(threads) as ex:
             list(ex.map(run, jobs))
     return out
+
+
+def stats(lenses, nmodel: int, nlens: int, x0: float, y0: float, dx: float, nx: int, ny: int, planes=PLANES,
+          threads: int = 1) -> tuple:
+    """Per-pixel mean and variance of each plane over the `nmodel` lens models of a batch (PAPER.md:101, :114:
+    "map variances" over the tested parameter combinations).  The paper gives no formula; reading R21
+    (DESIGN.md): POPULATION variance.  Plain two-pass definition, in the order written:
+        mean = (1/M) sum_m P_m ;   var = (1/M) sum_m (P_m - mean)^2
+    with every P_m produced by grid() above.  Returns (mean, var), dicts name -> [ny, nx]."""
+    a = _as_lenses(lenses)
+    assert len(a) == nmodel * nlens and nmodel >= 1
+    maps = [grid(a[m * nlens:(m + 1) * nlens], x0, y0, dx, nx, ny, planes=planes, threads=threads)
+            for m in range(nmodel)]
+    mean, var = {}, {}
+    with np.errstate(invalid="ignore", over="ignore"):
+        for n in planes:
+            s = np.zeros((ny, nx), dtype=np.float64)
+            for m in range(nmodel):
+                s = s + maps[m][n]
+            mean[n] = s / nmodel
+            q = np.zeros((ny, nx), dtype=np.float64)
+            for m in range(nmodel):
+                d = maps[m][n] - mean[n]
+                q = q + d * d
+            var[n] = q / nmodel
+    return mean, var

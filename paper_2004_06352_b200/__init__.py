@@ -7,7 +7,7 @@ missing -- there is no CPU fallback (and it never imports `oracle`).
 
 Names mirror the C ABI one to one:
     lh_grid_gradient, lh_grid_hessian, lh_lens_maps, lh_grid_gradient_batch,
-    lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_pack_model, lh_set_stream,
+    lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_grid_stats_batch, lh_pack_model, lh_set_stream,
     lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_fp64_issue_probe, lh_math_host_eval, lh_version
 Outputs may be torch CUDA tensors (float64, contiguous), anything with a
 `data_ptr()`, or raw integer device addresses.
@@ -67,6 +67,8 @@ def _load():
         L.lh_grid_eval.argtypes = [vp, ci, gp, op]
         L.lh_grid_eval_batch.argtypes = [vp, ci, ci, gp, op]
         L.lh_grid_eval_host.argtypes = [vp, ci, ci, gp, op]
+        L.lh_grid_stats_batch.argtypes = [vp, ci, ci, gp, op, op]
+        L.lh_grid_stats_batch.restype = ci
         L.lh_set_stream.argtypes = [vp]
         L.lh_pack_model.argtypes = [vp, ci, vp, vp]
         L.lh_pack_model.restype = ci
@@ -163,6 +165,17 @@ def lh_grid_eval_batch(lenses, nmodel, nlens, grid, **planes):
         raise ValueError("len(lenses) != nmodel*nlens")
     o = _outputs(planes, _dev_ptr)
     _check(_load().lh_grid_eval_batch(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(o)))
+
+
+def lh_grid_stats_batch(lenses, nmodel, nlens, grid, mean: dict, var: dict | None = None):
+    """mean / var: dicts plane name -> device tensor [ny, nx]; per-pixel mean and population variance over models."""
+    a, p, n = _lenses_ptr(lenses)
+    if n != nmodel * nlens:
+        raise ValueError("len(lenses) != nmodel*nlens")
+    om = _outputs(mean, _dev_ptr)
+    ov = _outputs(var, _dev_ptr) if var else None
+    _check(_load().lh_grid_stats_batch(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(om),
+                                       C.byref(ov) if ov is not None else None))
 
 
 def lh_grid_eval_host(lenses, nmodel, nlens, grid, **host_planes):

@@ -115,7 +115,9 @@ int check_device_ptr(const double *p, const char *name) {
 const char *PLANE_NAMES[NPLANES] = {"ax", "ay", "a11", "a12", "a22", "kappa", "gamma1", "gamma2", "mu"};
 
 // Validate + pack + launch.  `dev_out` are device planes (already checked).
-int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *dev_out[NPLANES]) {
+// `dev_m2` != nullptr selects the statistics mode: dev_out are mean planes, dev_m2 variance planes.
+int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *dev_out[NPLANES],
+                double **dev_m2 = nullptr) {
     // a1: pack on the host (validates; nothing is enqueued if any lens is rejected)
     try {
         ctx.h_table.resize((size_t)nmodel * (size_t)nlens);
@@ -154,7 +156,11 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     J.nmodel = nmodel;
     J.x0 = g->x0; J.y0 = g->y0; J.dx = g->dx;
     J.nx = g->nx; J.ny = g->ny;
-    for (int k = 0; k < NPLANES; ++k) J.out[k] = dev_out[k];
+    for (int k = 0; k < NPLANES; ++k) {
+        J.out[k] = dev_out[k];
+        J.m2[k] = dev_m2 ? dev_m2[k] : nullptr;
+    }
+    J.stats = dev_m2 ? 1 : 0;
     J.carry = ctx.d_carry;
     CU(lh::launch_eval(J, s, &ctx.launches));
     if (carry_need) {
@@ -234,6 +240,31 @@ int lh_grid_gradient_batch(const lh_lens *lenses, int nmodel, int nlens, const l
     std::memset(&o, 0, sizeof(o));
     o.ax = out_ax; o.ay = out_ay;
     return eval_checked(lenses, nmodel, nlens, g, &o);
+}
+
+int lh_grid_stats_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *mean,
+                        const lh_outputs *var) {
+    ctx.err[0] = 0;
+    int rc = check_common(lenses, nmodel, nlens, g);
+    if (rc) return rc;
+    if ((rc = check_grid(g, 1))) return rc;
+    if (!mean) return fail(LH_EINVAL, "lh_grid_stats_batch: mean is NULL");
+    double *pm[NPLANES], *pv[NPLANES];
+    planes_of(mean, pm);
+    for (int k = 0; k < NPLANES; ++k) pv[k] = nullptr;
+    if (var) planes_of(var, pv);
+    bool any = false;
+    for (int k = 0; k < NPLANES; ++k) {
+        if (pv[k] && !pm[k]) return fail(LH_EINVAL, "variance of %s requested without its mean", PLANE_NAMES[k]);
+        if (pm[k]) {
+            any = true;
+            if ((rc = check_device_ptr(pm[k], PLANE_NAMES[k]))) return rc;
+        }
+        if (pv[k] && (rc = check_device_ptr(pv[k], PLANE_NAMES[k]))) return rc;
+        if (pv[k] && pv[k] == pm[k]) return fail(LH_EINVAL, "mean and variance of %s share a buffer", PLANE_NAMES[k]);
+    }
+    if (!any) return fail(LH_EINVAL, "no output plane requested");
+    return eval_device(lenses, nmodel, nlens, g, pm, pv);
 }
 
 int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *host_o) {

@@ -323,6 +323,35 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
         v[7][k] = g2;
         v[8][k] = 1.0 / det;
     }
+    if (P.stats) {
+        // f2: running mean / variance over the models of a batch (Welford), one model per launch
+        // (blockIdx.y == 0), so a pixel is updated by exactly one thread per launch and launches
+        // are ordered by the stream.  n = models seen including this one.
+        const double n = (double)(P.model0 + 1);
+#pragma unroll
+        for (int pl = 0; pl < 9; ++pl) {
+            if ((pl < 2 && !GRAD) || (pl >= 2 && !HESS)) continue;
+            double *o = P.out[pl], *q = P.m2[pl];
+            if (o == nullptr) continue;
+#pragma unroll
+            for (int k = 0; k < PX; ++k) {
+                if (i0 + k >= P.nx) continue;
+                double mean = 0.0, m2 = 0.0;
+                if (P.model0 > 0) {
+                    mean = o[pix + k];
+                    if (q) m2 = q[pix + k];
+                }
+                const double d = v[pl][k] - mean;
+                mean += d / n;
+                o[pix + k] = mean;
+                if (q) {
+                    m2 = fma(d, v[pl][k] - mean, m2);
+                    q[pix + k] = (P.stats == 2) ? m2 / n : m2;
+                }
+            }
+        }
+        return;
+    }
 #pragma unroll
     for (int pl = 0; pl < 9; ++pl) {
         if ((pl < 2 && !GRAD) || (pl >= 2 && !HESS)) continue;
@@ -356,7 +385,8 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     Q.x0 = J.x0; Q.y0 = J.y0; Q.dx = J.dx;
     Q.nx = J.nx; Q.ny = J.ny;
     Q.plane = (long long)J.nx * J.ny;
-    for (int k = 0; k < 9; ++k) Q.out[k] = J.out[k];
+    for (int k = 0; k < 9; ++k) { Q.out[k] = J.out[k]; Q.m2[k] = J.stats ? J.m2[k] : nullptr; }
+    Q.stats = 0;
     Q.carry = J.carry;
     Q.math = J.math;
     Q.tiles_x = (J.nx + TILE_W - 1) / TILE_W;
@@ -383,7 +413,7 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     if (n <= LAUNCH_RECORDS) {
         // whole models per launch
         const int per = n > 0 ? LAUNCH_RECORDS / n : LAUNCH_MODELS;
-        const int mpl = per < LAUNCH_MODELS ? per : LAUNCH_MODELS;
+        const int mpl = J.stats ? 1 : (per < LAUNCH_MODELS ? per : LAUNCH_MODELS);  // stats: one model per launch
         for (int m0 = 0; m0 < J.nmodel; m0 += mpl) {
             const int nm = (J.nmodel - m0 < mpl) ? J.nmodel - m0 : mpl;
             bool extreme = false;
@@ -394,6 +424,7 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
             }
             if (n > 0) std::memcpy(Q.table, J.table + (size_t)m0 * n, (size_t)nm * n * sizeof(LensK));
             Q.model0 = m0; Q.stride = n; Q.first = 1; Q.last = 1;
+            if (J.stats) Q.stats = (m0 == J.nmodel - 1) ? 2 : 1;
             cudaError_t e = go(nm, extreme);
             if (e != cudaSuccess) return e;
         }
@@ -414,6 +445,7 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
             extreme = Q.cls_end[0][CLS_EXTREME] > Q.cls_end[0][CLS_SIS];
             std::memcpy(Q.table, J.table + (size_t)m * n + lo, (size_t)(hi - lo) * sizeof(LensK));
             Q.model0 = m; Q.stride = hi - lo; Q.first = (c == 0); Q.last = (c == nch - 1);
+            if (J.stats) Q.stats = (m == J.nmodel - 1) ? 2 : 1;
             cudaError_t e = go(1, extreme);
             if (e != cudaSuccess) return e;
         }

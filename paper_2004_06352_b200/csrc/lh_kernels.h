@@ -22,7 +22,9 @@ struct LaunchParams {
     int model0;              // global index of the launch's first model (blockIdx.y = model - model0)
     int stride;              // records per model in table[]
     int first, last;         // this launch holds the first / last lens chunk of its model(s)
-    int pad_;
+    int stats;               // 0: out[] are per-model planes.  1 / 2: out[] are running MEANS over models and m2[] the
+                             // running sums of squared deviations (Welford); 2 = last model: m2[] is divided by the count
+    double *m2[9];           // stats only; nullptr = variance of that plane not wanted
     unsigned short cls_end[LAUNCH_MODELS][CLS_COUNT];  // per model: end of each class, relative to its slice
     LensK table[LAUNCH_RECORDS];
 };
@@ -37,6 +39,8 @@ struct EvalJob {
     double x0, y0, dx;
     int nx, ny;
     double *out[9];  // DEVICE
+    double *m2[9];   // DEVICE, stats only (else all nullptr)
+    int stats;       // 0 = per-model planes [nmodel][ny][nx]; 1 = mean / variance over the models, planes [ny][nx]
     double *carry;   // DEVICE, 5*nx*ny doubles; needed only when nlens > LAUNCH_RECORDS
 };
 

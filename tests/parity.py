@@ -61,3 +61,22 @@ def check_planes(got: dict, ref: dict, what="", rel=REL):
     bad = {n: v for n, v in worst.items() if not v <= 1.0}
     assert not bad, f"{what}: parity violated (|d|/allowed): {bad}"
     return worst
+
+
+def stats_violation(mean_got, var_got, mean_ref, var_ref, nmodel: int):
+    """Mean / variance of a plane over the models of a batch (lh_grid_stats_batch vs oracle.stats; R21).
+
+    Each sample P_m is allowed the plain per-element error e = max(1e-11 |P_m|, 1e-13 max|plane|); per pixel
+    |P_m| <= |mean| + sqrt(M var), so e <= max(1e-11 (|mean| + sqrt(M var)), 1e-13 max|mean plane|) =: E.
+    mean: |d mean| <= E.   var = (1/M) sum (P_m - mean)^2: perturbing every sample by <= E moves it by at most
+    2 sqrt(var) (2E) + (2E)^2 (Cauchy-Schwarz; the factor 2 covers the shift of the mean), plus the rounding of the
+    sum itself, 1e-11 var.  Returns max |d| / allowed for (mean, var)."""
+    mean_ref = np.asarray(mean_ref, dtype=np.float64)
+    var_ref = np.asarray(var_ref, dtype=np.float64)
+    fin = np.isfinite(mean_ref) & np.isfinite(var_ref)
+    E = np.maximum(REL * (np.abs(mean_ref) + np.sqrt(nmodel * var_ref)), FLOOR * np.max(np.abs(mean_ref[fin])))
+    am = np.maximum(E, 5e-324)
+    av = 4.0 * np.sqrt(var_ref) * E + 4.0 * E * E + REL * var_ref
+    vm = float(np.max(np.abs(mean_got - mean_ref)[fin] / am[fin]))
+    vv = float(np.max(np.abs(var_got - var_ref)[fin] / np.maximum(av[fin], 5e-324)))
+    return vm, vv

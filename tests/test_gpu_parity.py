@@ -13,7 +13,7 @@ import pytest
 import lens_inputs as li
 import oracle
 import paper_2004_06352_b200 as lh
-from parity import check_planes, conditioned_rel, plain_violation
+from parity import check_planes, conditioned_rel, plain_violation, stats_violation
 
 pytestmark = pytest.mark.gpu
 
@@ -237,6 +237,70 @@ def test_far_field_and_large_scales():
     L[1] = (li.DPIE, 0, -3.0, 4.0, 0.6, 2.0, 1e-3, 2e-3, 1.0)  # rcut barely above rcore scale
     g = li.Grid(x0=-1e4, y0=-1e4, dx=157.3, nx=128, ny=128)
     check_planes(run_gpu(L, g, li.ALL_PLANES), ref_grid(L, g, li.ALL_PLANES), "far field")
+
+
+# ------------------------------------------------------------------ f2: map statistics over a batch
+def _stats_gpu(c, names, var_names):
+    g = c.grid
+    mean = dev_planes(names, (g.ny, g.nx))
+    var = dev_planes(var_names, (g.ny, g.nx))
+    lh.lh_grid_stats_batch(c.lenses, c.nmodel, c.nlens, g, mean, var)
+    torch.cuda.synchronize()
+    return {n: v.cpu().numpy() for n, v in mean.items()}, {n: v.cpu().numpy() for n, v in var.items()}
+
+
+def test_stats_cfg4_scaled_whole_maps():
+    """64 models x 300 lenses (two lens chunks per model) on 64 x 64: mean and variance of ax, ay, kappa, gamma1."""
+    c = li.config(4, scale=16)
+    names = ("ax", "ay", "kappa", "gamma1")
+    g = c.grid
+    mean, var = _stats_gpu(c, names, names)
+    rmean, rvar = oracle.stats(c.lenses, c.nmodel, c.nlens, g.x0, g.y0, g.dx, g.nx, g.ny, planes=names, threads=NTHREADS)
+    for n in names:
+        vm, vv = stats_violation(mean[n], var[n], rmean[n], rvar[n], c.nmodel)
+        assert vm <= 1.0 and vv <= 1.0, (n, vm, vv)
+        assert (var[n] >= 0).all()
+
+
+def test_stats_small_models_mean_only_and_single_model():
+    c = li.config(2)
+    rng = np.random.default_rng(11)
+    nmodel, nlens = 9, 12
+    L = c.lenses[rng.integers(0, len(c.lenses), nmodel * nlens)]
+    g = li.Grid(x0=-30.0, y0=-20.0, dx=0.9, nx=67, ny=9)
+    names = ("ax", "a11", "a12", "a22", "kappa", "gamma2")
+    mean = dev_planes(names, (g.ny, g.nx))
+    var = dev_planes(("kappa",), (g.ny, g.nx))
+    n0 = lh.lh_launch_count()
+    lh.lh_grid_stats_batch(L, nmodel, nlens, g, mean, var)
+    torch.cuda.synchronize()
+    assert lh.lh_launch_count() - n0 == nmodel  # statistics mode: one launch chain per model
+    rmean, rvar = oracle.stats(L, nmodel, nlens, g.x0, g.y0, g.dx, g.nx, g.ny, planes=names)
+    for n in names:
+        vm, _ = stats_violation(mean[n].cpu().numpy(), rvar[n], rmean[n], rvar[n], nmodel)
+        assert vm <= 1.0, (n, vm)
+    _, vv = stats_violation(rmean["kappa"], var["kappa"].cpu().numpy(), rmean["kappa"], rvar["kappa"], nmodel)
+    assert vv <= 1.0
+    # one model: mean is the map itself (bitwise), variance exactly zero
+    one = dev_planes(("ax", "kappa"), (g.ny, g.nx))
+    onev = dev_planes(("ax", "kappa"), (g.ny, g.nx))
+    lh.lh_grid_stats_batch(L[:nlens], 1, nlens, g, one, onev)
+    ref = run_gpu(L[:nlens], g, ("ax", "kappa"))
+    for n in ref:
+        assert np.array_equal(one[n].cpu().numpy(), ref[n]) and (onev[n] == 0).all()
+
+
+def test_stats_argument_errors():
+    c = li.config(0)
+    g = c.grid
+    k = dev_planes(("kappa",), (g.ny, g.nx))
+    with pytest.raises(lh.LhError):
+        lh.lh_grid_stats_batch(c.lenses, 1, c.nlens, g, {}, k)           # variance without its mean
+    with pytest.raises(lh.LhError):
+        lh.lh_grid_stats_batch(c.lenses, 1, c.nlens, g, k, k)            # shared buffer
+    with pytest.raises(lh.LhError):
+        lh.lh_grid_stats_batch(c.lenses, 1, c.nlens, g, {}, None)        # nothing requested
+    assert torch.isnan(k["kappa"]).all()
 
 
 # ------------------------------------------------------------------ ABI behaviour on the device
