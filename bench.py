@@ -64,6 +64,9 @@ def parse():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--stats", action="store_true",
+                    help="NEXT row f2 on a batch config (use --config 4): per-pixel mean and variance of ax ay kappa "
+                         "gamma1 gamma2 over the models through lh_grid_stats_batch (not the default bench line)")
     return ap.parse_args()
 
 
@@ -165,7 +168,8 @@ def workload_config(cfg, args):
     g = cfg.grid
     return {"workload": f"BASELINE.json configs[{args.config}] {cfg.name}: {g.nx}x{g.ny} px, {cfg.nlens} lenses"
                         + (f" x {cfg.nmodel} models" if cfg.nmodel > 1 else ""),
-            "outputs": list(cfg.outputs), "evals_per_step_per_gpu": cfg.evals,
+            "outputs": (["mean+variance over models of"] if getattr(args, "stats", False) else []) + list(cfg.outputs),
+            "evals_per_step_per_gpu": cfg.evals,
             "l2": "output planes (%d MiB/step) exceed the 126 MB L2 and a 256 MiB buffer is rewritten between "
                   "timed steps; the lens records (%d KiB) travel in the kernel parameters"
                   % (len(cfg.outputs) * cfg.nmodel * g.npix * 8 >> 20, cfg.nmodel * cfg.nlens * 192 >> 10),
@@ -197,13 +201,21 @@ def run_ours(args):
         lenses = li.cluster(1000 * args.config + rank, {1: 2, 2: 3, 3: 4}.get(args.config, 0), cfg.nlens
                             - {1: 2, 2: 3, 3: 4}.get(args.config, 0), {0: 40.0, 3: 150.0}.get(args.config, 100.0))
     shape = (cfg.nmodel, g.ny, g.nx)
+    if args.stats:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, outputs=("ax", "ay", "kappa", "gamma1", "gamma2"))
+        shape = (g.ny, g.nx)
+        var = {n: torch.empty(shape, dtype=torch.float64, device="cuda") for n in cfg.outputs}
     out = {n: torch.empty(shape, dtype=torch.float64, device="cuda") for n in cfg.outputs}
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
     lh.lh_set_stream(stream)
 
     def step():
-        lh.lh_grid_eval_batch(lenses, cfg.nmodel, cfg.nlens, g, **out)
+        if args.stats:
+            lh.lh_grid_stats_batch(lenses, cfg.nmodel, cfg.nlens, g, out, var)
+        else:
+            lh.lh_grid_eval_batch(lenses, cfg.nmodel, cfg.nlens, g, **out)
 
     def barrier():
         if world > 1:
@@ -238,8 +250,16 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         host = {n: torch.empty(shape, dtype=torch.float64).pin_memory() for n in cfg.outputs}
+        hvar = {n: torch.empty(shape, dtype=torch.float64).pin_memory() for n in cfg.outputs} if args.stats else None
         def step_host():
-            lh.lh_grid_eval_host(lenses, cfg.nmodel, cfg.nlens, g, **host)
+            if args.stats:  # host lens list in; mean and variance planes copied to pinned host memory
+                step()
+                for n in host:
+                    host[n].copy_(out[n], non_blocking=True)
+                    hvar[n].copy_(var[n], non_blocking=True)
+                torch.cuda.synchronize()
+            else:
+                lh.lh_grid_eval_host(lenses, cfg.nmodel, cfg.nlens, g, **host)
         step_host()
         barrier()
         t0 = time.perf_counter()
@@ -254,7 +274,8 @@ def run_ours(args):
             dt = float(t.item())
         e2e = {"value": world * cfg.evals * k_e2e / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(cfg.nmodel * cfg.nlens * 192 + cfg.nmodel * 8),
-               "d2h_bytes_per_step": int(len(cfg.outputs) * cfg.nmodel * g.npix * 8),
+               "d2h_bytes_per_step": int(len(cfg.outputs) * g.npix * 16 if args.stats else
+                                         len(cfg.outputs) * cfg.nmodel * g.npix * 8),
                "ms_per_step": 1e3 * dt / k_e2e, "steps": k_e2e,
                "note": "lh_grid_eval_host: host lens list in, pinned host planes out, packing + copies + sync timed"}
         del host
