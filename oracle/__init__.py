@@ -165,3 +165,37 @@ def stats(lenses, nmodel: int, nlens: int, x0: float, y0: float, dx: float, nx: 
                 q = q + d * d
             var[n] = q / nmodel
     return mean, var
+
+
+# ---------------------------------------------------------------- NEXT row f1: source plane, delensing
+ORC_IMAGE_DTYPE = np.dtype([("source", "<i4"), ("pad_", "<i4"), ("triangle", "<i8"), ("x", "<f8"), ("y", "<f8")])
+
+
+def source_plane(ax, ay, x0: float, y0: float, dx: float):
+    """beta = theta - alpha on the grid (eq. 1): returns (bx, by), each [ny, nx]."""
+    ax = np.ascontiguousarray(ax, dtype=np.float64)
+    ay = np.ascontiguousarray(ay, dtype=np.float64)
+    ny, nx = ax.shape
+    bx, by = np.empty_like(ax), np.empty_like(ay)
+    L = lib()
+    L.orc_source_plane.restype = None
+    L.orc_source_plane.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int,
+                                   C.c_void_p, C.c_void_p]
+    L.orc_source_plane(ax.ctypes.data, ay.ctypes.data, x0, y0, dx, nx, ny, bx.ctypes.data, by.ctypes.data)
+    return bx, by
+
+
+def delens(ax, ay, x0: float, y0: float, dx: float, sources, max_images: int = 1 << 20):
+    """Brute-force image search (readings R22): returns (images[ORC_IMAGE_DTYPE], found)."""
+    ax = np.ascontiguousarray(ax, dtype=np.float64)
+    ay = np.ascontiguousarray(ay, dtype=np.float64)
+    ny, nx = ax.shape
+    src = np.ascontiguousarray(sources, dtype=np.float64).reshape(-1, 2)
+    images = np.zeros(max_images, dtype=ORC_IMAGE_DTYPE)
+    L = lib()
+    L.orc_delens.restype = C.c_longlong
+    L.orc_delens.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.c_void_p,
+                             C.c_int, C.c_void_p, C.c_longlong]
+    found = L.orc_delens(ax.ctypes.data, ay.ctypes.data, x0, y0, dx, nx, ny, src.ctypes.data, len(src),
+                         images.ctypes.data, max_images)
+    return images[: min(found, max_images)], int(found)

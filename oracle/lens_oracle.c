@@ -219,3 +219,85 @@ void orc_grid_rows(const orc_lens *lenses, int nlens, double x0, double y0, doub
         }
     }
 }
+
+/*
+ * ---- NEXT row f1: source plane and brute-force delensing -----------------------------------
+ * Lens equation beta = theta - alpha(theta)                       PAPER.md:39 (eq. 1)
+ * "the 'brute force' approach is to unlens a image-plane grid unto the source-plane and check each
+ * quadrant for the presence of the source (see Fig.4)"            PAPER.md:87-91 (sec. 2.3)
+ * "searching for the images by delensing and checking the grid for sources ... Each image found is
+ * stored"                                                         PAPER.md:194 (sec. 4.2, stage 3)
+ * The paper gives no triangulation, inside rule or image position; readings R22:
+ *   - vertices are the grid pixels; cell (i, j), 0 <= i < nx-1, 0 <= j < ny-1, has the corners
+ *     V00 = (i, j), V10 = (i+1, j), V01 = (i, j+1), V11 = (i+1, j+1) and is cut along V10-V01 into
+ *     triangle 0 = (V00, V10, V01) and triangle 1 = (V11, V01, V10); triangle id = 2*(j*(nx-1)+i)+t;
+ *   - with A, B, C the triangle's vertices mapped to the source plane and S the source,
+ *     d = (B-A) x (C-A), u = (S-A) x (C-A) / d, v = (B-A) x (S-A) / d; the source is inside iff
+ *     d != 0, u >= 0, v >= 0 and u + v <= 1 (closed triangle: a source exactly on a shared edge is
+ *     reported by both neighbours);
+ *   - the image is the same barycentric combination of the image-plane vertices:
+ *     theta = tA + u (tB - tA) + v (tC - tA).
+ * Images are emitted in triangle order, sources in index order inside a triangle.
+ */
+typedef struct {
+    int32_t source;   /* index into the source list */
+    int32_t pad_;
+    int64_t triangle; /* 2*(j*(nx-1)+i) + t */
+    double x, y;      /* image position in the image plane */
+} orc_image;
+
+void orc_source_plane(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,
+                      double *bx, double *by) {
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            const size_t p = (size_t)j * (size_t)nx + (size_t)i;
+            bx[p] = (x0 + (double)i * dx) - ax[p];
+            by[p] = (y0 + (double)j * dx) - ay[p];
+        }
+}
+
+static int tri_test(const double A[2], const double B[2], const double C[2], const double S[2], double *u, double *v) {
+    const double e1x = B[0] - A[0], e1y = B[1] - A[1];
+    const double e2x = C[0] - A[0], e2y = C[1] - A[1];
+    const double sx = S[0] - A[0], sy = S[1] - A[1];
+    const double d = e1x * e2y - e1y * e2x;
+    if (d == 0.0) return 0;
+    *u = (sx * e2y - sy * e2x) / d;
+    *v = (e1x * sy - e1y * sx) / d;
+    return *u >= 0.0 && *v >= 0.0 && *u + *v <= 1.0;
+}
+
+/* returns the number of images found (may exceed max_images; only the first max_images are stored) */
+long long orc_delens(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,
+                     const double *sources /* [ns][2] */, int ns, orc_image *images, long long max_images) {
+    long long found = 0;
+    for (int j = 0; j + 1 < ny; ++j)
+        for (int i = 0; i + 1 < nx; ++i) {
+            double T[4][2], Bq[4][2]; /* 00, 10, 01, 11: image-plane and source-plane corners */
+            for (int c = 0; c < 4; ++c) {
+                const int ii = i + (c & 1), jj = j + (c >> 1);
+                const size_t p = (size_t)jj * (size_t)nx + (size_t)ii;
+                T[c][0] = x0 + (double)ii * dx;
+                T[c][1] = y0 + (double)jj * dx;
+                Bq[c][0] = T[c][0] - ax[p];
+                Bq[c][1] = T[c][1] - ay[p];
+            }
+            static const int V[2][3] = {{0, 1, 2}, {3, 2, 1}};
+            for (int t = 0; t < 2; ++t)
+                for (int s = 0; s < ns; ++s) {
+                    double u, v;
+                    const int a = V[t][0], b = V[t][1], c = V[t][2];
+                    if (!tri_test(Bq[a], Bq[b], Bq[c], &sources[2 * s], &u, &v)) continue;
+                    if (found < max_images) {
+                        orc_image *im = &images[found];
+                        im->source = s;
+                        im->pad_ = 0;
+                        im->triangle = 2 * ((int64_t)j * (nx - 1) + i) + t;
+                        im->x = T[a][0] + u * (T[b][0] - T[a][0]) + v * (T[c][0] - T[a][0]);
+                        im->y = T[a][1] + u * (T[b][1] - T[a][1]) + v * (T[c][1] - T[a][1]);
+                    }
+                    ++found;
+                }
+        }
+    return found;
+}
