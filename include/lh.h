@@ -125,6 +125,35 @@ int lh_grid_eval_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_gr
 int lh_grid_stats_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *mean,
                         const lh_outputs *var);
 
+/* ---- NEXT row f1: source plane and brute-force delensing ------------------------------------------------
+ * Source-plane position of every grid pixel, beta = theta - alpha(theta) (eq. 1), from deflection
+ * planes already on the device.  ax, ay, bx, by: DEVICE [ny][nx]; bx or by may be NULL (not wanted); bx / by may
+ * alias ax / ay (in place).  Errors as lh_grid_gradient. */
+int lh_source_plane(const double *ax, const double *ay, const lh_grid *g, double *bx, double *by);
+
+/* One predicted image. */
+typedef struct {
+    int32_t source;   /* index into `sources` */
+    int32_t _pad;     /* 0 */
+    int64_t triangle; /* 2*(j*(nx-1)+i) + t: cell (i, j), t = 0 for (V00, V10, V01), 1 for (V11, V01, V10) */
+    double x, y;      /* image-plane position */
+} lh_image;
+
+/* Brute-force image search: "unlens a image-plane grid unto the source-plane and check each quadrant for the
+ * presence of the source" (sec. 2.3, Fig. 4; stage 3 of the chi^2 computation).
+ * The grid pixels are the vertices; every cell is cut along V10-V01 into two triangles; a triangle whose
+ * source-plane image contains source s (closed triangle, barycentric test) yields one image at the same
+ * barycentric combination of its image-plane vertices (readings R22).
+ *   ax, ay     DEVICE [ny][nx] deflection planes (e.g. from lh_grid_gradient on the same grid)
+ *   sources    HOST [nsources][2] source-plane positions, read during the call
+ *   images     DEVICE, room for max_images records; the ORDER of the records is not defined
+ *   count      DEVICE; set to the number of images FOUND, which may exceed max_images (then only
+ *              max_images records were stored)
+ * Asynchronous on the set stream.  LH_EINVAL: NULL pointer, nsources < 0, max_images < 0, bad grid, pointer
+ * that is not device memory. */
+int lh_delens_grid(const double *ax, const double *ay, const lh_grid *g, const double *sources, int nsources,
+                   lh_image *images, long long max_images, long long *count);
+
 /* Same as lh_grid_eval_batch with HOST output planes: the library allocates (and
  * caches) device planes, runs the same kernel, copies the requested planes back
  * and synchronises the stream before returning.  This is the end-to-end path a

@@ -69,6 +69,10 @@ def _load():
         L.lh_grid_eval_host.argtypes = [vp, ci, ci, gp, op]
         L.lh_grid_stats_batch.argtypes = [vp, ci, ci, gp, op, op]
         L.lh_grid_stats_batch.restype = ci
+        L.lh_source_plane.argtypes = [dp, dp, gp, dp, dp]
+        L.lh_source_plane.restype = ci
+        L.lh_delens_grid.argtypes = [dp, dp, gp, vp, ci, vp, C.c_longlong, vp]
+        L.lh_delens_grid.restype = ci
         L.lh_set_stream.argtypes = [vp]
         L.lh_pack_model.argtypes = [vp, ci, vp, vp]
         L.lh_pack_model.restype = ci
@@ -176,6 +180,26 @@ def lh_grid_stats_batch(lenses, nmodel, nlens, grid, mean: dict, var: dict | Non
     ov = _outputs(var, _dev_ptr) if var else None
     _check(_load().lh_grid_stats_batch(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(om),
                                        C.byref(ov) if ov is not None else None))
+
+
+LH_IMAGE_DTYPE = np.dtype([("source", "<i4"), ("_pad", "<i4"), ("triangle", "<i8"), ("x", "<f8"), ("y", "<f8")])
+
+
+def lh_source_plane(ax, ay, grid, bx=None, by=None):
+    """beta = theta - alpha on the grid; device planes [ny, nx]."""
+    _check(_load().lh_source_plane(_dev_ptr(ax), _dev_ptr(ay), C.byref(_grid(grid)), _dev_ptr(bx), _dev_ptr(by)))
+
+
+def lh_delens_grid(ax, ay, grid, sources, images, max_images: int, count):
+    """sources: host float64 [ns, 2]; images: device buffer of >= max_images 32-byte lh_image records (e.g. a
+    torch uint8 tensor of 32*max_images bytes, view it with LH_IMAGE_DTYPE on the host); count: device int64[1]."""
+    src = np.ascontiguousarray(sources, dtype=np.float64).reshape(-1, 2)
+
+    def raw(t):  # any device buffer: only the address is taken
+        return None if t is None else (t if isinstance(t, int) else t.data_ptr())
+
+    _check(_load().lh_delens_grid(_dev_ptr(ax), _dev_ptr(ay), C.byref(_grid(grid)), src.ctypes.data, len(src),
+                                  raw(images), int(max_images), raw(count)))
 
 
 def lh_grid_eval_host(lenses, nmodel, nlens, grid, **host_planes):

@@ -13,6 +13,12 @@
 #include "../../include/lh.h"
 #include "lh_kernels.h"
 
+namespace lh {
+cudaError_t launch_delens(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,
+                          const double *sources, int ns, lh_image *images, long long max_images,
+                          unsigned long long *count, int sms, cudaStream_t st, long long *launches);
+}
+
 namespace {
 
 using lh::LensK;
@@ -265,6 +271,46 @@ int lh_grid_stats_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_g
     }
     if (!any) return fail(LH_EINVAL, "no output plane requested");
     return eval_device(lenses, nmodel, nlens, g, pm, pv);
+}
+
+int lh_source_plane(const double *ax, const double *ay, const lh_grid *g, double *bx, double *by) {
+    ctx.err[0] = 0;
+    int rc = check_grid(g, 1);
+    if (rc) return rc;
+    if (!ax || !ay) return fail(LH_EINVAL, "lh_source_plane: ax and ay are required");
+    if (!bx && !by) return fail(LH_EINVAL, "no output plane requested");
+    if ((rc = check_device_ptr(ax, "ax")) || (rc = check_device_ptr(ay, "ay"))) return rc;
+    if (bx && (rc = check_device_ptr(bx, "bx"))) return rc;
+    if (by && (rc = check_device_ptr(by, "by"))) return rc;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CU(lh::launch_source_plane(ax, ay, g->x0, g->y0, g->dx, g->nx, g->ny, bx, by, sms, ctx.stream));
+    ++ctx.launches;
+    return LH_OK;
+}
+
+int lh_delens_grid(const double *ax, const double *ay, const lh_grid *g, const double *sources, int nsources,
+                   lh_image *images, long long max_images, long long *count) {
+    ctx.err[0] = 0;
+    int rc = check_grid(g, 1);
+    if (rc) return rc;
+    if (!ax || !ay || !count) return fail(LH_EINVAL, "lh_delens_grid: ax, ay and count are required");
+    if (nsources < 0 || max_images < 0) return fail(LH_EINVAL, "lh_delens_grid: nsources and max_images must be >= 0");
+    if (nsources > 0 && !sources) return fail(LH_EINVAL, "sources is NULL");
+    if (max_images > 0 && !images) return fail(LH_EINVAL, "images is NULL");
+    if ((rc = check_device_ptr(ax, "ax")) || (rc = check_device_ptr(ay, "ay"))) return rc;
+    if ((rc = check_device_ptr(reinterpret_cast<const double *>(count), "count"))) return rc;
+    if (images && (rc = check_device_ptr(reinterpret_cast<const double *>(images), "images"))) return rc;
+    for (int s = 0; s < 2 * nsources; ++s)
+        if (!std::isfinite(sources[s])) return fail(LH_EINVAL, "source %d: non-finite position", s / 2);
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CU(cudaMemsetAsync(count, 0, sizeof(long long), ctx.stream));
+    CU(lh::launch_delens(ax, ay, g->x0, g->y0, g->dx, g->nx, g->ny, sources, nsources, images, max_images,
+                         reinterpret_cast<unsigned long long *>(count), sms, ctx.stream, &ctx.launches));
+    return LH_OK;
 }
 
 int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *host_o) {

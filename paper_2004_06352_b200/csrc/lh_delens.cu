@@ -1,0 +1,137 @@
+// lh_delens.cu -- NEXT row f1: source-plane map and brute-force delensing (R22).
+//
+//   beta = theta - alpha(theta)                                         PAPER.md:39 (eq. 1)
+//   "unlens a image-plane grid unto the source-plane and check each quadrant for the presence of the
+//    source (see Fig.4)"                                                PAPER.md:87-91 (sec. 2.3)
+//   "searching for the images by delensing and checking the grid for sources ... Each image found is
+//    stored ... divergent execution path"                               PAPER.md:194 (sec. 4.2)
+//
+// One thread owns one grid cell (two triangles, cut along V10-V01).  The sources of a launch
+// travel in the kernel parameters, so the source index is warp-uniform and each source reaches the
+// comparisons as a uniform operand; a cell first rejects a source against the bounding box of its
+// four source-plane corners (the common, convergent path) and only then runs the exact barycentric
+// test.  The test arithmetic is written with the round-to-nearest intrinsics, i.e. WITHOUT FMA
+// contraction: it takes an integer decision (inside / outside) and must take it in exactly the
+// arithmetic the definition states, so that a triangle id never depends on the compiler.
+// Found images are appended through one atomic counter (order is not defined).
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "../../include/lh.h"
+#include "lh_kernels.h"
+
+namespace lh {
+
+constexpr int DELENS_SOURCES = 1024;  // sources per launch (16 KB of the 32 KB parameter space)
+constexpr int DELENS_THREADS = 256;
+
+struct DelensParams {
+    const double *ax, *ay;
+    lh_image *images;
+    unsigned long long *count;
+    long long max_images;
+    double x0, y0, dx;
+    int nx, ny;
+    int source0, nsources;  // global index of src[0]; sources in this launch
+    double src[DELENS_SOURCES][2];
+};
+static_assert(sizeof(DelensParams) <= 32764, "kernel parameter space");
+
+__device__ __forceinline__ double cross_rn(double ax, double ay, double bx, double by) {
+    return __dsub_rn(__dmul_rn(ax, by), __dmul_rn(ay, bx));
+}
+
+__device__ __forceinline__ void test_triangle(const DelensParams &P, int s, double sx, double sy, const double (&T)[4][2],
+                                              const double (&B)[4][2], int a, int b, int c, long long tri) {
+    const double e1x = __dsub_rn(B[b][0], B[a][0]), e1y = __dsub_rn(B[b][1], B[a][1]);
+    const double e2x = __dsub_rn(B[c][0], B[a][0]), e2y = __dsub_rn(B[c][1], B[a][1]);
+    const double px = __dsub_rn(sx, B[a][0]), py = __dsub_rn(sy, B[a][1]);
+    const double d = cross_rn(e1x, e1y, e2x, e2y);
+    if (d == 0.0) return;
+    const double u = __ddiv_rn(cross_rn(px, py, e2x, e2y), d);
+    const double v = __ddiv_rn(cross_rn(e1x, e1y, px, py), d);
+    if (!(u >= 0.0 && v >= 0.0 && __dadd_rn(u, v) <= 1.0)) return;
+    const unsigned long long k = atomicAdd(P.count, 1ULL);
+    if (k >= (unsigned long long)P.max_images) return;
+    lh_image im;
+    im.source = P.source0 + s;
+    im._pad = 0;
+    im.triangle = tri;
+    im.x = __dadd_rn(__dadd_rn(T[a][0], __dmul_rn(u, __dsub_rn(T[b][0], T[a][0]))), __dmul_rn(v, __dsub_rn(T[c][0], T[a][0])));
+    im.y = __dadd_rn(__dadd_rn(T[a][1], __dmul_rn(u, __dsub_rn(T[b][1], T[a][1]))), __dmul_rn(v, __dsub_rn(T[c][1], T[a][1])));
+    P.images[k] = im;
+}
+
+__global__ void __launch_bounds__(DELENS_THREADS) delens_kernel(const __grid_constant__ DelensParams P) {
+    const long long ncx = P.nx - 1, ncells = ncx * (P.ny - 1);
+    for (long long cell = (long long)blockIdx.x * DELENS_THREADS + threadIdx.x; cell < ncells;
+         cell += (long long)gridDim.x * DELENS_THREADS) {
+        const int j = (int)(cell / ncx), i = (int)(cell - (long long)j * ncx);
+        double T[4][2], B[4][2];  // corners 00, 10, 01, 11 in the image plane and in the source plane
+        double lox = 1e300, hix = -1e300, loy = 1e300, hiy = -1e300;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int ii = i + (c & 1), jj = j + (c >> 1);
+            const size_t p = (size_t)jj * P.nx + ii;
+            T[c][0] = __dadd_rn(P.x0, __dmul_rn((double)ii, P.dx));
+            T[c][1] = __dadd_rn(P.y0, __dmul_rn((double)jj, P.dx));
+            B[c][0] = __dsub_rn(T[c][0], __ldg(P.ax + p));
+            B[c][1] = __dsub_rn(T[c][1], __ldg(P.ay + p));
+            lox = fmin(lox, B[c][0]); hix = fmax(hix, B[c][0]);
+            loy = fmin(loy, B[c][1]); hiy = fmax(hiy, B[c][1]);
+        }
+        for (int s = 0; s < P.nsources; ++s) {
+            const double sx = P.src[s][0], sy = P.src[s][1];
+            // a point of a closed triangle lies inside the bounding box of its vertices: exact reject
+            if (sx < lox || sx > hix || sy < loy || sy > hiy) continue;
+            test_triangle(P, s, sx, sy, T, B, 0, 1, 2, 2 * cell);
+            test_triangle(P, s, sx, sy, T, B, 3, 2, 1, 2 * cell + 1);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) source_plane_kernel(const double *__restrict__ ax, const double *__restrict__ ay,
+                                                           double x0, double y0, double dx, int nx, int ny,
+                                                           double *__restrict__ bx, double *__restrict__ by) {
+    const long long n = (long long)nx * ny;
+    for (long long p = (long long)blockIdx.x * 256 + threadIdx.x; p < n; p += (long long)gridDim.x * 256) {
+        const int j = (int)(p / nx), i = (int)(p - (long long)j * nx);
+        if (bx) bx[p] = __dsub_rn(__dadd_rn(x0, __dmul_rn((double)i, dx)), ax[p]);
+        if (by) by[p] = __dsub_rn(__dadd_rn(y0, __dmul_rn((double)j, dx)), ay[p]);
+    }
+}
+
+cudaError_t launch_source_plane(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,
+                                double *bx, double *by, int sms, cudaStream_t st) {
+    const long long n = (long long)nx * ny;
+    long long blocks = (n + 255) / 256;
+    if (blocks > (long long)sms * 16) blocks = (long long)sms * 16;
+    source_plane_kernel<<<(unsigned)blocks, 256, 0, st>>>(ax, ay, x0, y0, dx, nx, ny, bx, by);
+    return cudaGetLastError();
+}
+
+// sources: HOST [ns][2].  One launch per DELENS_SOURCES sources; `count` must be zero on entry.
+cudaError_t launch_delens(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,
+                          const double *sources, int ns, lh_image *images, long long max_images,
+                          unsigned long long *count, int sms, cudaStream_t st, long long *launches) {
+    thread_local DelensParams P;
+    P.ax = ax; P.ay = ay; P.images = images; P.count = count; P.max_images = max_images;
+    P.x0 = x0; P.y0 = y0; P.dx = dx; P.nx = nx; P.ny = ny;
+    const long long ncells = (long long)(nx - 1) * (ny - 1);
+    if (ncells <= 0) return cudaSuccess;
+    long long blocks = (ncells + DELENS_THREADS - 1) / DELENS_THREADS;
+    if (blocks > (long long)sms * 8) blocks = (long long)sms * 8;  // persistent: 8 CTAs of 256 threads per SM
+    for (int s0 = 0; s0 < ns; s0 += DELENS_SOURCES) {
+        const int n = ns - s0 < DELENS_SOURCES ? ns - s0 : DELENS_SOURCES;
+        P.source0 = s0; P.nsources = n;
+        for (int s = 0; s < n; ++s) { P.src[s][0] = sources[2 * (s0 + s)]; P.src[s][1] = sources[2 * (s0 + s) + 1]; }
+        delens_kernel<<<(unsigned)blocks, DELENS_THREADS, 0, st>>>(P);
+        ++*launches;
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+}  // namespace lh

@@ -49,4 +49,8 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
 cudaError_t launch_dfma_probe(int iters, int blocks, double *sink, cudaStream_t stream);
 cudaError_t launch_issue_probe(int variant, int extra, int iters, int blocks, double *sink, cudaStream_t stream);  // lh_probe.cu
 
+// lh_delens.cu (NEXT row f1)
+cudaError_t launch_source_plane(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,
+                                double *bx, double *by, int sms, cudaStream_t st);
+
 }  // namespace lh
