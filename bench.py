@@ -64,6 +64,9 @@ def parse():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--delens", action="store_true",
+                    help="NEXT row f1 alone (not the default bench line): lh_delens_grid on the deflection planes of "
+                         "--config (default 3) for 80 synthetic sources (M1149 has 80, PAPER.md:208)")
     ap.add_argument("--stats", action="store_true",
                     help="NEXT row f2 on a batch config (use --config 4): per-pixel mean and variance of ax ay kappa "
                          "gamma1 gamma2 over the models through lh_grid_stats_batch (not the default bench line)")
@@ -328,8 +331,72 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_delens(args):
+    """f1 measured alone: one step = lh_delens_grid over the whole grid for 80 sources (deflection planes resident)."""
+    import torch
+
+    import paper_2004_06352_b200 as lh
+
+    torch.cuda.set_device(0)
+    cfg = li.config(args.config)
+    g = cfg.grid
+    ax = torch.empty((g.ny, g.nx), dtype=torch.float64, device="cuda")
+    ay = torch.empty_like(ax)
+    stream = torch.cuda.current_stream()
+    lh.lh_set_stream(stream)
+    lh.lh_grid_gradient(cfg.lenses[: cfg.nlens], g, ax, ay)
+    ns = 80
+    rng = np.random.default_rng(1234)
+    half = 0.3 * g.nx * g.dx / 2
+    src = np.column_stack([rng.uniform(-half, half, ns), rng.uniform(-half, half, ns)])
+    cap = 1 << 16
+    images = torch.zeros(32 * cap, dtype=torch.uint8, device="cuda")
+    count = torch.zeros(1, dtype=torch.int64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for _ in range(max(args.warmup, 3)):
+        lh.lh_delens_grid(ax, ay, g, src, images, cap, count)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    n0 = lh.lh_launch_count()
+    with ClockSampler(0) as clk:
+        for a, b in ev:
+            flush.zero_()
+            a.record(stream)
+            lh.lh_delens_grid(ax, ay, g, src, images, cap, count)
+            b.record(stream)
+        torch.cuda.synchronize()
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    cells = (g.nx - 1) * (g.ny - 1)
+    t0 = time.perf_counter()
+    import oracle
+    rows = 256  # bounded oracle sample: the first 256 rows of cells
+    hax, hay = ax[: rows + 1].cpu().numpy(), ay[: rows + 1].cpu().numpy()
+    t0 = time.perf_counter()
+    oracle.delens(hax, hay, g.x0, g.y0, g.dx, src)
+    dt = time.perf_counter() - t0
+    line = {"metric": "triangulated-grid delensing, cell-source tests/sec", "value": cells * ns / (ms * 1e-3),
+            "unit": "cell-source tests/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "images_found": int(count.item()),
+            "config": {"workload": f"NEXT row f1: {g.nx}x{g.ny} vertices of configs[{args.config}], {ns} sources"},
+            "clocks": clk.summary(), "gpu_launches": int(lh.lh_launch_count() - n0),
+            "roofline": {"bound": "alu", "achieved": cells * ns / (ms * 1e-3) / 1e12, "peak": 148 * 64 * 1.965e9 / 4 / 1e12,
+                         "unit": "T cell-source tests/s", "frac": cells * ns / (ms * 1e-3) / (148 * 64 * 1.965e9 / 4),
+                         "traffic": None,
+                         "note": "the common path of a (cell, source) pair is the exact bounding-box reject = 4 FP64 "
+                                 "compares; peak = 148 SM x 64 FP64 lanes x 1.965 GHz / 4.  HBM side: the two "
+                                 "deflection planes are read once (16 B per vertex) = %.0f GB/s of the measured 6545"
+                                 % (16.0 * g.npix / (ms * 1e-3) / 1e9)},
+            "cpu_baseline": {"value": rows * (g.nx - 1) * ns / dt, "unit": "cell-source tests/s", "cores": 1,
+                             "kind": "oracle", "sample": f"first {rows} cell rows, {ns} sources, {dt:.1f} s"}}
+    print(json.dumps(line), flush=True)
+
+
 if __name__ == "__main__":
     a = parse()
+    if a.delens and a.impl != "reference":
+        run_delens(a)
+        raise SystemExit(0)
     if a.impl == "reference":
         run_reference(a)
     else:
