@@ -39,6 +39,9 @@
  *              output element has been written; lh_last_error() gives a message.
  *              No exception or abort crosses this boundary.
  *   nlens = 0  is valid: alpha = 0, a_ij = 0, kappa = gamma = 0, mu = 1.
+ *   range      lengths (positions, radii, pixel size) may use any unit, but all of them must lie within about
+ *              1e+-35 of one another: the kernel takes ONE reciprocal of a product of four squared lengths
+ *              per evaluation and that product must stay inside the double range.
  *   IEEE       mu = +-inf where det A^-1 == 0 exactly.  A pixel that coincides
  *              exactly with the centre of an SIS gets zero contribution from it.
  */
