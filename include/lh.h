@@ -117,6 +117,14 @@ int lh_grid_eval(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_ou
 /* Batched form of lh_grid_eval (layout as lh_grid_gradient_batch). */
 int lh_grid_eval_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *o);
 
+/* Batch whose models share most of their lenses (NEXT row f4): model m = `shared` (nshared lenses, the same for
+ * every model -- e.g. the cluster galaxies an MCMC step leaves untouched) + varying[m*nvar .. (m+1)*nvar).  The
+ * shared lenses are superposed ONCE; every model starts from those sums (the superposition is linear, PAPER.md:183
+ * eq. 10, :112).  Result and layout as lh_grid_eval_batch on the concatenated lists (summation order differs).
+ * nvar <= 160 when nshared > 0; nvar = 0 and nshared = 0 are valid.  Errors as lh_grid_gradient. */
+int lh_grid_eval_batch_shared(const lh_lens *shared, int nshared, const lh_lens *varying, int nmodel, int nvar,
+                              const lh_grid *g, const lh_outputs *o);
+
 /* Per-pixel MEAN and VARIANCE of the requested planes over the `nmodel` lens models of a batch -- the
  * statistical-error maps of the Bayesian process: "In order to compute the map variances, full-resolution
  * lensing maps have to be generated for each tested parameter-combination" (sec. 2.4; 10014 maps

@@ -69,6 +69,8 @@ def _load():
         L.lh_grid_eval_host.argtypes = [vp, ci, ci, gp, op]
         L.lh_grid_stats_batch.argtypes = [vp, ci, ci, gp, op, op]
         L.lh_grid_stats_batch.restype = ci
+        L.lh_grid_eval_batch_shared.argtypes = [vp, ci, vp, ci, ci, gp, op]
+        L.lh_grid_eval_batch_shared.restype = ci
         L.lh_source_plane.argtypes = [dp, dp, gp, dp, dp]
         L.lh_source_plane.restype = ci
         L.lh_delens_grid.argtypes = [dp, dp, gp, vp, ci, vp, C.c_longlong, vp]
@@ -169,6 +171,16 @@ def lh_grid_eval_batch(lenses, nmodel, nlens, grid, **planes):
         raise ValueError("len(lenses) != nmodel*nlens")
     o = _outputs(planes, _dev_ptr)
     _check(_load().lh_grid_eval_batch(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(o)))
+
+
+def lh_grid_eval_batch_shared(shared, varying, nmodel, nvar, grid, **planes):
+    """model m = shared + varying[m*nvar:(m+1)*nvar]; planes [nmodel, ny, nx]; the shared lenses are evaluated once."""
+    sa, sp, sn = _lenses_ptr(shared)
+    va, vpn, vn = _lenses_ptr(varying)
+    if vn != nmodel * nvar:
+        raise ValueError("len(varying) != nmodel*nvar")
+    o = _outputs(planes, _dev_ptr)
+    _check(_load().lh_grid_eval_batch_shared(sp, sn, vpn, nmodel, nvar, C.byref(_grid(grid)), C.byref(o)))
 
 
 def lh_grid_stats_batch(lenses, nmodel, nlens, grid, mean: dict, var: dict | None = None):

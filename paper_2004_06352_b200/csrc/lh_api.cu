@@ -35,7 +35,7 @@ struct Context {
     char err[512] = {0};
     long long launches = 0;
 
-    std::vector<LensK> h_table;
+    std::vector<LensK> h_table, h_shared;
     std::vector<ModelRanges> h_ranges;
 
     double *d_carry = nullptr;
@@ -122,8 +122,9 @@ const char *PLANE_NAMES[NPLANES] = {"ax", "ay", "a11", "a12", "a22", "kappa", "g
 
 // Validate + pack + launch.  `dev_out` are device planes (already checked).
 // `dev_m2` != nullptr selects the statistics mode: dev_out are mean planes, dev_m2 variance planes.
+// `shared` != nullptr: lenses common to every model (f4), evaluated once.
 int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *dev_out[NPLANES],
-                double **dev_m2 = nullptr) {
+                double **dev_m2 = nullptr, const lh_lens *shared = nullptr, int nshared = 0) {
     // a1: pack on the host (validates; nothing is enqueued if any lens is rejected)
     try {
         ctx.h_table.resize((size_t)nmodel * (size_t)nlens);
@@ -137,9 +138,21 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
             return LH_EINVAL;  // message already written
     }
 
+    lh::ModelRanges shared_ranges = {};
+    if (nshared > 0) {
+        try {
+            ctx.h_shared.resize((size_t)nshared);
+        } catch (const std::bad_alloc &) {
+            return fail(LH_EINVAL, "out of host memory packing %d shared lenses", nshared);
+        }
+        if (lh::pack_model(shared, nshared, ctx.h_shared.data(), &shared_ranges, ctx.err, sizeof(ctx.err), -1) != 0)
+            return LH_EINVAL;
+    }
+
     cudaStream_t s = ctx.stream;
     if (!ctx.ev_done) CU(cudaEventCreateWithFlags(&ctx.ev_done, cudaEventDisableTiming));
-    const size_t carry_need = nlens > lh::LAUNCH_RECORDS ? (size_t)5 * g->nx * g->ny * sizeof(double) : 0;
+    const size_t carry_need =
+        (nlens > lh::LAUNCH_RECORDS || nshared > 0) ? (size_t)5 * g->nx * g->ny * sizeof(double) : 0;
     if (carry_need > ctx.carry_bytes) {
         if (ctx.busy) CU(cudaEventSynchronize(ctx.ev_done));  // the old buffer is no longer in use
         if (ctx.d_carry) cudaFree(ctx.d_carry);
@@ -160,6 +173,9 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     J.ranges = ctx.h_ranges.data();
     J.nlens = nlens;
     J.nmodel = nmodel;
+    J.shared_table = nshared > 0 ? ctx.h_shared.data() : nullptr;
+    J.shared_ranges = shared_ranges;
+    J.nshared = nshared;
     J.x0 = g->x0; J.y0 = g->y0; J.dx = g->dx;
     J.nx = g->nx; J.ny = g->ny;
     for (int k = 0; k < NPLANES; ++k) {
@@ -246,6 +262,28 @@ int lh_grid_gradient_batch(const lh_lens *lenses, int nmodel, int nlens, const l
     std::memset(&o, 0, sizeof(o));
     o.ax = out_ax; o.ay = out_ay;
     return eval_checked(lenses, nmodel, nlens, g, &o);
+}
+
+int lh_grid_eval_batch_shared(const lh_lens *shared, int nshared, const lh_lens *varying, int nmodel, int nvar,
+                              const lh_grid *g, const lh_outputs *o) {
+    ctx.err[0] = 0;
+    int rc = check_common(varying, nmodel, nvar, g);
+    if (rc) return rc;
+    if (nshared < 0 || (nshared > 0 && !shared)) return fail(LH_EINVAL, "shared lens list: bad argument");
+    if (nshared >= (1 << 30)) return fail(LH_EINVAL, "nshared must be < 2^30");
+    if (nshared > 0 && nvar > lh::LAUNCH_RECORDS)
+        return fail(LH_EINVAL, "at most %d varying lenses per model beside a shared list", lh::LAUNCH_RECORDS);
+    if (!o) return fail(LH_EINVAL, "outputs is NULL");
+    double *p[NPLANES];
+    planes_of(o, p);
+    bool any = false;
+    for (int k = 0; k < NPLANES; ++k) {
+        if (!p[k]) continue;
+        any = true;
+        if ((rc = check_device_ptr(p[k], PLANE_NAMES[k]))) return rc;
+    }
+    if (!any) return fail(LH_EINVAL, "no output plane requested");
+    return eval_device(varying, nmodel, nvar, g, p, nullptr, shared, nshared);
 }
 
 int lh_grid_stats_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *mean,

@@ -410,6 +410,32 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     };
 
     const int n = J.nlens;
+    // lens chunks [lo, hi) of one packed model -> consecutive launches of a single model slot
+    auto chunks = [&](const LensK *table, const ModelRanges &rg, int count, int model, bool first_is_first, bool last_is_last,
+                      int stats) -> cudaError_t {
+        const int nch = (count + LAUNCH_RECORDS - 1) / LAUNCH_RECORDS;
+        for (int c = 0; c < nch; ++c) {
+            const int lo = (int)((long long)count * c / nch), hi = (int)((long long)count * (c + 1) / nch);
+            for (int k = 0; k < CLS_COUNT; ++k) {
+                int e = rg.begin[k + 1] - lo;
+                e = e < 0 ? 0 : (e > hi - lo ? hi - lo : e);
+                Q.cls_end[0][k] = (unsigned short)e;
+            }
+            const bool extreme = Q.cls_end[0][CLS_EXTREME] > Q.cls_end[0][CLS_SIS];
+            std::memcpy(Q.table, table + lo, (size_t)(hi - lo) * sizeof(LensK));
+            Q.model0 = model; Q.stride = hi - lo;
+            Q.first = (c == 0) && first_is_first; Q.last = (c == nch - 1) && last_is_last;
+            Q.stats = stats;
+            cudaError_t e = go(1, extreme);
+            if (e != cudaSuccess) return e;
+        }
+        return cudaSuccess;
+    };
+    const bool shared = J.nshared > 0;
+    if (shared) {  // f4: the common lenses once, left in `carry` (never reaches the epilogue)
+        cudaError_t e = chunks(J.shared_table, J.shared_ranges, J.nshared, 0, true, false, 0);
+        if (e != cudaSuccess) return e;
+    }
     if (n <= LAUNCH_RECORDS) {
         // whole models per launch
         const int per = n > 0 ? LAUNCH_RECORDS / n : LAUNCH_MODELS;
@@ -423,32 +449,18 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
                 extreme = extreme || rg.begin[CLS_EXTREME + 1] > rg.begin[CLS_EXTREME];
             }
             if (n > 0) std::memcpy(Q.table, J.table + (size_t)m0 * n, (size_t)nm * n * sizeof(LensK));
-            Q.model0 = m0; Q.stride = n; Q.first = 1; Q.last = 1;
-            if (J.stats) Q.stats = (m0 == J.nmodel - 1) ? 2 : 1;
+            Q.model0 = m0; Q.stride = n; Q.first = shared ? 0 : 1; Q.last = 1;
+            Q.stats = J.stats ? ((m0 == J.nmodel - 1) ? 2 : 1) : 0;
             cudaError_t e = go(nm, extreme);
             if (e != cudaSuccess) return e;
         }
         return cudaSuccess;
     }
     // one model at a time, balanced lens chunks
-    const int nch = (n + LAUNCH_RECORDS - 1) / LAUNCH_RECORDS;
     for (int m = 0; m < J.nmodel; ++m) {
-        const ModelRanges &rg = J.ranges[m];
-        for (int c = 0; c < nch; ++c) {
-            const int lo = (int)((long long)n * c / nch), hi = (int)((long long)n * (c + 1) / nch);
-            bool extreme = false;
-            for (int k = 0; k < CLS_COUNT; ++k) {
-                int e = rg.begin[k + 1] - lo;
-                e = e < 0 ? 0 : (e > hi - lo ? hi - lo : e);
-                Q.cls_end[0][k] = (unsigned short)e;
-            }
-            extreme = Q.cls_end[0][CLS_EXTREME] > Q.cls_end[0][CLS_SIS];
-            std::memcpy(Q.table, J.table + (size_t)m * n + lo, (size_t)(hi - lo) * sizeof(LensK));
-            Q.model0 = m; Q.stride = hi - lo; Q.first = (c == 0); Q.last = (c == nch - 1);
-            if (J.stats) Q.stats = (m == J.nmodel - 1) ? 2 : 1;
-            cudaError_t e = go(1, extreme);
-            if (e != cudaSuccess) return e;
-        }
+        cudaError_t e = chunks(J.table + (size_t)m * n, J.ranges[m], n, m, true, true,
+                               J.stats ? ((m == J.nmodel - 1) ? 2 : 1) : 0);
+        if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
 }

@@ -36,6 +36,11 @@ struct EvalJob {
     const ModelRanges *ranges;  // HOST [nmodel]
     const MathTables *math;     // DEVICE
     int nlens, nmodel;
+    // f4: lenses common to every model of the batch, evaluated ONCE into `carry`; every model then starts from
+    // those accumulators (nullptr / 0 = none).  Needs nlens <= LAUNCH_RECORDS and carry != nullptr.
+    const LensK *shared_table;  // HOST [nshared], sorted by class
+    ModelRanges shared_ranges;
+    int nshared;
     double x0, y0, dx;
     int nx, ny;
     double *out[9];  // DEVICE

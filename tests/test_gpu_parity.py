@@ -239,6 +239,55 @@ def test_far_field_and_large_scales():
     check_planes(run_gpu(L, g, li.ALL_PLANES), ref_grid(L, g, li.ALL_PLANES), "far field")
 
 
+# ------------------------------------------------------------------ f4: batches that share most of their lenses
+def test_shared_lens_batch_cfg4_scaled():
+    """cfg 4 keeps the 298 galaxies fixed and perturbs the 2 halos: shared = galaxies (two lens chunks, evaluated
+    once), varying = 2 halos per model.  Must match the oracle on every model's full 300-lens list."""
+    c = li.config(4, scale=16)
+    g = c.grid
+    L = c.lenses.reshape(c.nmodel, c.nlens)
+    shared, varying = L[0, 2:].copy(), np.ascontiguousarray(L[:, :2]).reshape(-1)
+    assert all(np.array_equal(L[m, 2:], shared) for m in range(c.nmodel))
+    names = ("ax", "ay", "kappa", "gamma1", "mu")
+    out = dev_planes(names, (c.nmodel, g.ny, g.nx))
+    n0 = lh.lh_launch_count()
+    lh.lh_grid_eval_batch_shared(shared, varying, c.nmodel, 2, g, **out)
+    torch.cuda.synchronize()
+    assert lh.lh_launch_count() - n0 == 2 + 1  # 298 shared lenses in two chunks + 64 x 2 varying in one launch
+    for m in range(0, c.nmodel, 7):
+        ref = ref_grid(c.lenses[m * c.nlens:(m + 1) * c.nlens], g, names)
+        check_planes({n: out[n][m].cpu().numpy() for n in names}, ref, f"shared batch model {m}")
+
+
+def test_shared_lens_batch_edge_cases():
+    c = li.config(2)
+    g = li.Grid(x0=-30.0, y0=-20.0, dx=0.9, nx=67, ny=9)
+    shared = c.lenses[:40]  # dPIE + NSIE + SIS
+    # nvar = 0: every model is the shared list
+    out = dev_planes(("ax", "kappa"), (3, g.ny, g.nx))
+    lh.lh_grid_eval_batch_shared(shared, li.make_lenses(0), 3, 0, g, **out)
+    ref = ref_grid(shared, g, ("ax", "kappa"))
+    for m in range(3):
+        check_planes({n: out[n][m].cpu().numpy() for n in out}, ref, "nvar=0")
+    # nshared = 0: plain batch, bitwise
+    var = c.lenses[40:52]
+    a = dev_planes(("ay", "mu"), (3, g.ny, g.nx))
+    b = dev_planes(("ay", "mu"), (3, g.ny, g.nx))
+    lh.lh_grid_eval_batch_shared(li.make_lenses(0), var, 3, 4, g, **a)
+    lh.lh_grid_eval_batch(var, 3, 4, g, **b)
+    torch.cuda.synchronize()
+    assert all(torch.equal(a[n], b[n]) for n in a)
+    # too many varying lenses beside a shared list, bad lens in the shared list: nothing written
+    o = dev_planes(("ax",), (1, g.ny, g.nx))
+    with pytest.raises(lh.LhError):
+        lh.lh_grid_eval_batch_shared(shared, c.lenses[:161], 1, 161, g, **o)
+    bad = shared.copy()
+    bad["rcore"][0] = -1.0
+    with pytest.raises(lh.LhError):
+        lh.lh_grid_eval_batch_shared(bad, var, 3, 4, g, **dev_planes(("ax",), (3, g.ny, g.nx)))
+    assert torch.isnan(o["ax"]).all()
+
+
 # ------------------------------------------------------------------ f2: map statistics over a batch
 def _stats_gpu(c, names, var_names):
     g = c.grid
