@@ -280,7 +280,8 @@ def run_ours(args):
                "d2h_bytes_per_step": int(len(cfg.outputs) * g.npix * 16 if args.stats else
                                          len(cfg.outputs) * cfg.nmodel * g.npix * 8),
                "ms_per_step": 1e3 * dt / k_e2e, "steps": k_e2e,
-               "note": "lh_grid_eval_host: host lens list in, pinned host planes out, packing + copies + sync timed"}
+               "note": "lh_grid_eval_host: host lens list in, pinned host planes out, packing + copies + sync timed; "
+                       "the D2H copy of each of 8 row slabs overlaps the computation of the next"}
         del host
 
     if rank != 0:

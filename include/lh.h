@@ -167,7 +167,10 @@ int lh_delens_grid(const double *ax, const double *ay, const lh_grid *g, const d
 
 /* Same as lh_grid_eval_batch with HOST output planes: the library allocates (and
  * caches) device planes, runs the same kernel, copies the requested planes back
- * and synchronises the stream before returning.  This is the end-to-end path a
+ * and synchronises the stream before returning.  Large jobs are cut into up to 8
+ * pieces (row slabs of one map, groups of models of a batch) so that the copy of one
+ * piece overlaps the computation of the next; the results are bit-identical to the
+ * device entry point's.  This is the end-to-end path a
  * caller without device buffers uses. */
 int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *host_o);
 

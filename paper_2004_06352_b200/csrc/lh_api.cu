@@ -46,6 +46,9 @@ struct Context {
 
     double *d_planes = nullptr;  // cached device planes for the *_host entry point
     size_t planes_bytes = 0;
+    static const int PIECES = 8;  // pipeline depth of the *_host entry point (compute piece k+1 | copy piece k)
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_piece[PIECES] = {};
     double *d_sink = nullptr;
 
     ~Context() {
@@ -124,7 +127,10 @@ const char *PLANE_NAMES[NPLANES] = {"ax", "ay", "a11", "a12", "a22", "kappa", "g
 // `dev_m2` != nullptr selects the statistics mode: dev_out are mean planes, dev_m2 variance planes.
 // `shared` != nullptr: lenses common to every model (f4), evaluated once.
 int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *dev_out[NPLANES],
-                double **dev_m2 = nullptr, const lh_lens *shared = nullptr, int nshared = 0) {
+                double **dev_m2 = nullptr, const lh_lens *shared = nullptr, int nshared = 0, int j0 = 0,
+                int nrows = -1) {
+    // rows [j0, j0 + nrows) of the grid only (dev_out then point at row j0 of every plane); default: all rows
+    if (nrows < 0) nrows = g->ny;
     // a1: pack on the host (validates; nothing is enqueued if any lens is rejected)
     try {
         ctx.h_table.resize((size_t)nmodel * (size_t)nlens);
@@ -177,13 +183,15 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     J.shared_ranges = shared_ranges;
     J.nshared = nshared;
     J.x0 = g->x0; J.y0 = g->y0; J.dx = g->dx;
-    J.nx = g->nx; J.ny = g->ny;
+    J.nx = g->nx; J.ny = nrows;
+    J.j0 = j0;
+    J.plane = (long long)g->nx * g->ny;
     for (int k = 0; k < NPLANES; ++k) {
         J.out[k] = dev_out[k];
         J.m2[k] = dev_m2 ? dev_m2[k] : nullptr;
     }
     J.stats = dev_m2 ? 1 : 0;
-    J.carry = ctx.d_carry;
+    J.carry = ctx.d_carry ? ctx.d_carry + (size_t)j0 * g->nx : nullptr;
     CU(lh::launch_eval(J, s, &ctx.launches));
     if (carry_need) {
         CU(cudaEventRecord(ctx.ev_done, s));
@@ -376,10 +384,39 @@ int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_gri
     int slot = 0;
     for (int k = 0; k < NPLANES; ++k)
         dp[k] = hp[k] ? ctx.d_planes + (size_t)(slot++) * (plane_bytes / sizeof(double)) : nullptr;
-    rc = eval_device(lenses, nmodel, nlens, g, dp);
-    if (rc) return rc;
-    for (int k = 0; k < NPLANES; ++k)
-        if (hp[k]) CU(cudaMemcpyAsync(hp[k], dp[k], plane_bytes, cudaMemcpyDeviceToHost, ctx.stream));
+
+    // Pipeline: the work is cut into pieces (row slabs of one map, or groups of models of a batch); the
+    // device-to-host copy of piece k runs on a second stream while piece k+1 is being computed.
+    if (!ctx.copy_stream) {
+        CU(cudaStreamCreateWithFlags(&ctx.copy_stream, cudaStreamNonBlocking));
+        for (int k = 0; k < Context::PIECES; ++k) CU(cudaEventCreateWithFlags(&ctx.ev_piece[k], cudaEventDisableTiming));
+    }
+    const size_t npix = (size_t)g->nx * g->ny;
+    const int units = nmodel == 1 ? g->ny : nmodel;  // rows or models
+    // small jobs are not worth cutting: about 4 MB of results per piece at least
+    long long want = (long long)(need >> 22);
+    const int pieces = want < 1 ? 1 : (want > Context::PIECES ? Context::PIECES : (int)want);
+    int per = (units + pieces - 1) / pieces;
+    if (nmodel == 1) per = (per + 7) & ~7;            // whole pixel tiles
+    int piece = 0;
+    for (int u0 = 0; u0 < units; u0 += per, ++piece) {
+        const int nu = units - u0 < per ? units - u0 : per;
+        double *sub[NPLANES];
+        const size_t off = nmodel == 1 ? (size_t)u0 * g->nx : (size_t)u0 * npix;
+        const size_t count = nmodel == 1 ? (size_t)nu * g->nx : (size_t)nu * npix;
+        for (int k = 0; k < NPLANES; ++k) sub[k] = dp[k] ? dp[k] + off : nullptr;
+        rc = nmodel == 1 ? eval_device(lenses, 1, nlens, g, sub, nullptr, nullptr, 0, u0, nu)
+                         : eval_device(lenses + (size_t)u0 * nlens, nu, nlens, g, sub);
+        if (rc) {
+            cudaStreamSynchronize(ctx.copy_stream);
+            return rc;  // a lens was rejected on the first piece: nothing enqueued, nothing written
+        }
+        CU(cudaEventRecord(ctx.ev_piece[piece], ctx.stream));
+        CU(cudaStreamWaitEvent(ctx.copy_stream, ctx.ev_piece[piece], 0));
+        for (int k = 0; k < NPLANES; ++k)
+            if (hp[k]) CU(cudaMemcpyAsync(hp[k] + off, dp[k] + off, count * sizeof(double), cudaMemcpyDeviceToHost, ctx.copy_stream));
+    }
+    CU(cudaStreamSynchronize(ctx.copy_stream));
     CU(cudaStreamSynchronize(ctx.stream));
     return LH_OK;
 }

@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
     double X[PX];
 #pragma unroll
     for (int k = 0; k < PX; ++k) X[k] = fma((double)(i0 + k), P.dx, P.x0);
-    const double Y = fma((double)j, P.dx, P.y0);
+    const double Y = fma((double)(j + P.j0), P.dx, P.y0);
 
     const int m = blockIdx.y;  // model inside this launch
     const size_t pix = (size_t)j * P.nx + i0;
@@ -384,7 +384,8 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     thread_local LaunchParams Q;  // 32 KB: kept off the stack
     Q.x0 = J.x0; Q.y0 = J.y0; Q.dx = J.dx;
     Q.nx = J.nx; Q.ny = J.ny;
-    Q.plane = (long long)J.nx * J.ny;
+    Q.plane = J.plane;
+    Q.j0 = J.j0;
     for (int k = 0; k < 9; ++k) { Q.out[k] = J.out[k]; Q.m2[k] = J.stats ? J.m2[k] : nullptr; }
     Q.stats = 0;
     Q.carry = J.carry;

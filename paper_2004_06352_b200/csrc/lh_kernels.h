@@ -18,7 +18,8 @@ struct LaunchParams {
     double *out[9];          // ax ay a11 a12 a22 kappa gamma1 gamma2 mu; nullptr = not wanted; [nmodel][ny][nx]
     double *carry;           // [5][ny][nx] accumulators handed from one lens chunk of a model to the next
     const MathTables *math;  // device copy of the atan / atanh reduction tables
-    int nx, ny, tiles_x;
+    int nx, ny, tiles_x;     // ny = rows of THIS launch (a row slab of the grid when j0 > 0)
+    int j0;                  // first grid row of the slab: pixel row j of the launch sits at y0 + (j0 + j) dx
     int model0;              // global index of the launch's first model (blockIdx.y = model - model0)
     int stride;              // records per model in table[]
     int first, last;         // this launch holds the first / last lens chunk of its model(s)
@@ -42,7 +43,9 @@ struct EvalJob {
     ModelRanges shared_ranges;
     int nshared;
     double x0, y0, dx;
-    int nx, ny;
+    int nx, ny;      // ny = rows evaluated by this job
+    int j0;          // first grid row (row slab of a larger grid; out[] / carry already point at that row)
+    long long plane; // doubles between consecutive models / accumulators (the FULL plane, >= nx*ny)
     double *out[9];  // DEVICE
     double *m2[9];   // DEVICE, stats only (else all nullptr)
     int stats;       // 0 = per-model planes [nmodel][ny][nx]; 1 = mean / variance over the models, planes [ny][nx]
