@@ -114,6 +114,13 @@ int lh_grid_gradient_batch(const lh_lens *lenses, int nmodel, int nlens, const l
  * must be non-NULL).  The four calls above are thin wrappers of this one. */
 int lh_grid_eval(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_outputs *o);
 
+/* Rows [j0, j0 + nrows) of the grid only -- the multi-GPU primitive: pixels are independent ("no need for
+ * communication between the different parallel tasks"; the paper splits the grid among its GPUs,
+ * PAPER.md:194), so each device evaluates a row slab with the whole lens list and no exchange.  The planes of
+ * `o` hold nrows*nx doubles (row j0 first).  Pixel coordinates are those of the full grid, so the slab is
+ * bit-identical to the same rows of lh_grid_eval.  0 <= j0, nrows >= 1, j0 + nrows <= ny. */
+int lh_grid_eval_rows(const lh_lens *lenses, int nlens, const lh_grid *g, int j0, int nrows, const lh_outputs *o);
+
 /* Batched form of lh_grid_eval (layout as lh_grid_gradient_batch). */
 int lh_grid_eval_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *o);
 

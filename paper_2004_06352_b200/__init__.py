@@ -69,6 +69,8 @@ def _load():
         L.lh_grid_eval_host.argtypes = [vp, ci, ci, gp, op]
         L.lh_grid_stats_batch.argtypes = [vp, ci, ci, gp, op, op]
         L.lh_grid_stats_batch.restype = ci
+        L.lh_grid_eval_rows.argtypes = [vp, ci, gp, ci, ci, op]
+        L.lh_grid_eval_rows.restype = ci
         L.lh_grid_eval_batch_shared.argtypes = [vp, ci, vp, ci, ci, gp, op]
         L.lh_grid_eval_batch_shared.restype = ci
         L.lh_source_plane.argtypes = [dp, dp, gp, dp, dp]
@@ -163,6 +165,13 @@ def lh_grid_eval(lenses, grid, **planes):
     a, p, n = _lenses_ptr(lenses)
     o = _outputs(planes, _dev_ptr)
     _check(_load().lh_grid_eval(p, n, C.byref(_grid(grid)), C.byref(o)))
+
+
+def lh_grid_eval_rows(lenses, grid, j0: int, nrows: int, **planes):
+    """Rows [j0, j0+nrows) of the grid into planes of shape [nrows, nx] (the multi-GPU row-slab primitive)."""
+    a, p, n = _lenses_ptr(lenses)
+    o = _outputs(planes, _dev_ptr)
+    _check(_load().lh_grid_eval_rows(p, n, C.byref(_grid(grid)), int(j0), int(nrows), C.byref(o)))
 
 
 def lh_grid_eval_batch(lenses, nmodel, nlens, grid, **planes):

@@ -191,7 +191,9 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
         J.m2[k] = dev_m2 ? dev_m2[k] : nullptr;
     }
     J.stats = dev_m2 ? 1 : 0;
-    J.carry = ctx.d_carry ? ctx.d_carry + (size_t)j0 * g->nx : nullptr;
+    // carry is laid out like the planes it serves: a slab of FULL-size planes (nrows < g->ny) uses the slab's rows
+    // of a full-size carry; a stand-alone slab (lh_grid_eval_rows: g->ny == nrows) uses a carry of its own size
+    J.carry = ctx.d_carry ? ctx.d_carry + (nrows != g->ny ? (size_t)j0 * g->nx : 0) : nullptr;
     CU(lh::launch_eval(J, s, &ctx.launches));
     if (carry_need) {
         CU(cudaEventRecord(ctx.ev_done, s));
@@ -232,6 +234,27 @@ extern "C" {
 
 int lh_grid_eval(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_outputs *o) {
     return eval_checked(lenses, 1, nlens, g, o);
+}
+
+int lh_grid_eval_rows(const lh_lens *lenses, int nlens, const lh_grid *g, int j0, int nrows, const lh_outputs *o) {
+    ctx.err[0] = 0;
+    int rc = check_common(lenses, 1, nlens, g);
+    if (rc) return rc;
+    if (j0 < 0 || nrows < 1 || (long long)j0 + nrows > g->ny) return fail(LH_EINVAL, "row slab outside the grid");
+    if (!o) return fail(LH_EINVAL, "outputs is NULL");
+    double *p[NPLANES];
+    planes_of(o, p);
+    bool any = false;
+    for (int k = 0; k < NPLANES; ++k) {
+        if (!p[k]) continue;
+        any = true;
+        if ((rc = check_device_ptr(p[k], PLANE_NAMES[k]))) return rc;
+    }
+    if (!any) return fail(LH_EINVAL, "no output plane requested");
+    // the slab planes are stand-alone buffers: present them as a grid of nrows rows whose row 0 is grid row j0
+    lh_grid slab = *g;
+    slab.ny = nrows;
+    return eval_device(lenses, 1, nlens, &slab, p, nullptr, nullptr, 0, j0, nrows);
 }
 
 int lh_grid_eval_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *o) {
