@@ -121,6 +121,12 @@ int lh_grid_eval(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_ou
  * bit-identical to the same rows of lh_grid_eval.  0 <= j0, nrows >= 1, j0 + nrows <= ny. */
 int lh_grid_eval_rows(const lh_lens *lenses, int nlens, const lh_grid *g, int j0, int nrows, const lh_outputs *o);
 
+/* The same superposition at ARBITRARY points instead of a grid: xs, ys DEVICE [npoints]; every requested plane of
+ * `o` holds npoints doubles.  (Stage 2 of the paper's chi^2 pipeline unlenses the observed images, which are not
+ * on the grid: PAPER.md:76 Fig. 3, :192.)  Same kernels, same arithmetic; errors as lh_grid_gradient. */
+int lh_points_eval(const lh_lens *lenses, int nlens, const double *xs, const double *ys, long long npoints,
+                   const lh_outputs *o);
+
 /* Batched form of lh_grid_eval (layout as lh_grid_gradient_batch). */
 int lh_grid_eval_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *o);
 

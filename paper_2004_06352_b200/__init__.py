@@ -69,6 +69,8 @@ def _load():
         L.lh_grid_eval_host.argtypes = [vp, ci, ci, gp, op]
         L.lh_grid_stats_batch.argtypes = [vp, ci, ci, gp, op, op]
         L.lh_grid_stats_batch.restype = ci
+        L.lh_points_eval.argtypes = [vp, ci, dp, dp, C.c_longlong, op]
+        L.lh_points_eval.restype = ci
         L.lh_grid_eval_rows.argtypes = [vp, ci, gp, ci, ci, op]
         L.lh_grid_eval_rows.restype = ci
         L.lh_grid_eval_batch_shared.argtypes = [vp, ci, vp, ci, ci, gp, op]
@@ -165,6 +167,16 @@ def lh_grid_eval(lenses, grid, **planes):
     a, p, n = _lenses_ptr(lenses)
     o = _outputs(planes, _dev_ptr)
     _check(_load().lh_grid_eval(p, n, C.byref(_grid(grid)), C.byref(o)))
+
+
+def lh_points_eval(lenses, xs, ys, **planes):
+    """xs, ys: device float64 tensors of equal length; planes: device tensors of that length."""
+    a, p, n = _lenses_ptr(lenses)
+    npts = int(xs.numel()) if hasattr(xs, "numel") else None
+    if npts is None or npts != int(ys.numel()):
+        raise ValueError("xs and ys must be device tensors of equal length")
+    o = _outputs(planes, _dev_ptr)
+    _check(_load().lh_points_eval(p, n, _dev_ptr(xs), _dev_ptr(ys), npts, C.byref(o)))
 
 
 def lh_grid_eval_rows(lenses, grid, j0: int, nrows: int, **planes):

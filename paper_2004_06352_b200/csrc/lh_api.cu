@@ -124,12 +124,21 @@ int check_device_ptr(const double *p, const char *name) {
 const char *PLANE_NAMES[NPLANES] = {"ax", "ay", "a11", "a12", "a22", "kappa", "gamma1", "gamma2", "mu"};
 
 // Validate + pack + launch.  `dev_out` are device planes (already checked).
-// `dev_m2` != nullptr selects the statistics mode: dev_out are mean planes, dev_m2 variance planes.
-// `shared` != nullptr: lenses common to every model (f4), evaluated once.
+// Optional parts of a job.
+struct EvalOpts {
+    double **m2 = nullptr;            // != nullptr selects the statistics mode: dev_out are mean planes, m2 variance planes
+    const lh_lens *shared = nullptr;  // lenses common to every model (f4), evaluated once
+    int nshared = 0;
+    int j0 = 0, nrows = -1;           // rows [j0, j0 + nrows) of the grid only (dev_out point at row j0); default all
+    const double *px = nullptr, *py = nullptr;  // DEVICE: evaluate at these g->nx points instead of a grid (g->ny = 1)
+};
+
 int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *dev_out[NPLANES],
-                double **dev_m2 = nullptr, const lh_lens *shared = nullptr, int nshared = 0, int j0 = 0,
-                int nrows = -1) {
-    // rows [j0, j0 + nrows) of the grid only (dev_out then point at row j0 of every plane); default: all rows
+                const EvalOpts &opt = EvalOpts()) {
+    double **dev_m2 = opt.m2;
+    const lh_lens *shared = opt.shared;
+    const int nshared = opt.nshared, j0 = opt.j0;
+    int nrows = opt.nrows;
     if (nrows < 0) nrows = g->ny;
     // a1: pack on the host (validates; nothing is enqueued if any lens is rejected)
     try {
@@ -186,6 +195,7 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     J.nx = g->nx; J.ny = nrows;
     J.j0 = j0;
     J.plane = (long long)g->nx * g->ny;
+    J.px = opt.px; J.py = opt.py;
     for (int k = 0; k < NPLANES; ++k) {
         J.out[k] = dev_out[k];
         J.m2[k] = dev_m2 ? dev_m2[k] : nullptr;
@@ -254,7 +264,33 @@ int lh_grid_eval_rows(const lh_lens *lenses, int nlens, const lh_grid *g, int j0
     // the slab planes are stand-alone buffers: present them as a grid of nrows rows whose row 0 is grid row j0
     lh_grid slab = *g;
     slab.ny = nrows;
-    return eval_device(lenses, 1, nlens, &slab, p, nullptr, nullptr, 0, j0, nrows);
+    EvalOpts opt;
+    opt.j0 = j0; opt.nrows = nrows;
+    return eval_device(lenses, 1, nlens, &slab, p, opt);
+}
+
+int lh_points_eval(const lh_lens *lenses, int nlens, const double *xs, const double *ys, long long npoints,
+                   const lh_outputs *o) {
+    ctx.err[0] = 0;
+    if (npoints < 1 || npoints > 0x7fffffffLL) return fail(LH_EINVAL, "npoints must be in [1, 2^31)");
+    if (!xs || !ys) return fail(LH_EINVAL, "lh_points_eval: xs and ys are required");
+    lh_grid g = {0.0, 0.0, 1.0, (int32_t)npoints, 1};  // one row of "pixels"; the coordinates come from xs, ys
+    int rc = check_common(lenses, 1, nlens, &g);
+    if (rc) return rc;
+    if ((rc = check_device_ptr(xs, "xs")) || (rc = check_device_ptr(ys, "ys"))) return rc;
+    if (!o) return fail(LH_EINVAL, "outputs is NULL");
+    double *p[NPLANES];
+    planes_of(o, p);
+    bool any = false;
+    for (int k = 0; k < NPLANES; ++k) {
+        if (!p[k]) continue;
+        any = true;
+        if ((rc = check_device_ptr(p[k], PLANE_NAMES[k]))) return rc;
+    }
+    if (!any) return fail(LH_EINVAL, "no output plane requested");
+    EvalOpts opt;
+    opt.px = xs; opt.py = ys;
+    return eval_device(lenses, 1, nlens, &g, p, opt);
 }
 
 int lh_grid_eval_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *o) {
@@ -314,7 +350,9 @@ int lh_grid_eval_batch_shared(const lh_lens *shared, int nshared, const lh_lens 
         if ((rc = check_device_ptr(p[k], PLANE_NAMES[k]))) return rc;
     }
     if (!any) return fail(LH_EINVAL, "no output plane requested");
-    return eval_device(varying, nmodel, nvar, g, p, nullptr, shared, nshared);
+    EvalOpts opt;
+    opt.shared = shared; opt.nshared = nshared;
+    return eval_device(varying, nmodel, nvar, g, p, opt);
 }
 
 int lh_grid_stats_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *mean,
@@ -339,7 +377,9 @@ int lh_grid_stats_batch(const lh_lens *lenses, int nmodel, int nlens, const lh_g
         if (pv[k] && pv[k] == pm[k]) return fail(LH_EINVAL, "mean and variance of %s share a buffer", PLANE_NAMES[k]);
     }
     if (!any) return fail(LH_EINVAL, "no output plane requested");
-    return eval_device(lenses, nmodel, nlens, g, pm, pv);
+    EvalOpts opt;
+    opt.m2 = pv;
+    return eval_device(lenses, nmodel, nlens, g, pm, opt);
 }
 
 int lh_source_plane(const double *ax, const double *ay, const lh_grid *g, double *bx, double *by) {
@@ -428,7 +468,9 @@ int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_gri
         const size_t off = nmodel == 1 ? (size_t)u0 * g->nx : (size_t)u0 * npix;
         const size_t count = nmodel == 1 ? (size_t)nu * g->nx : (size_t)nu * npix;
         for (int k = 0; k < NPLANES; ++k) sub[k] = dp[k] ? dp[k] + off : nullptr;
-        rc = nmodel == 1 ? eval_device(lenses, 1, nlens, g, sub, nullptr, nullptr, 0, u0, nu)
+        EvalOpts opt;
+        if (nmodel == 1) { opt.j0 = u0; opt.nrows = nu; }
+        rc = nmodel == 1 ? eval_device(lenses, 1, nlens, g, sub, opt)
                          : eval_device(lenses + (size_t)u0 * nlens, nu, nlens, g, sub);
         if (rc) {
             cudaStreamSynchronize(ctx.copy_stream);

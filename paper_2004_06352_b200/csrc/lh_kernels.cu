@@ -225,7 +225,8 @@ __device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc
 template <bool GRAD, bool HESS>
 constexpr int min_blocks() { return (GRAD && HESS) ? LH_MINB : (GRAD ? LH_MINB_GRAD : LH_MINB_HESS); }
 
-template <bool GRAD, bool HESS, bool EXTREME>
+// POINTS: the "pixels" are arbitrary points (P.px[i], P.py[i]), one row of them, instead of a regular grid.
+template <bool GRAD, bool HESS, bool EXTREME, bool POINTS>
 __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>()) superpose_kernel(const __grid_constant__ LaunchParams P) {
     __shared__ SmemTables tb;
 
@@ -243,10 +244,20 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
     const bool inside = j < P.ny && i0 < P.nx;
 
     // a2: pixel coordinates from the grid definition (no coordinate array in memory)
-    double X[PX];
-#pragma unroll
-    for (int k = 0; k < PX; ++k) X[k] = fma((double)(i0 + k), P.dx, P.x0);
+    // (in grid mode every Yk[k] is the same value, so the row-wise subexpressions of the lens algebra are shared)
+    double X[PX], Yk[PX];
     const double Y = fma((double)(j + P.j0), P.dx, P.y0);
+#pragma unroll
+    for (int k = 0; k < PX; ++k) {
+        if (POINTS) {
+            const bool in = inside && i0 + k < P.nx;
+            X[k] = in ? __ldg(P.px + i0 + k) : 0.0;
+            Yk[k] = in ? __ldg(P.py + i0 + k) : 0.0;
+        } else {
+            X[k] = fma((double)(i0 + k), P.dx, P.x0);
+            Yk[k] = Y;
+        }
+    }
 
     const int m = blockIdx.y;  // model inside this launch
     const size_t pix = (size_t)j * P.nx + i0;
@@ -274,21 +285,21 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
     const int e2 = b + P.cls_end[m][2];  // end of SIS
     for (int l = b; l < e0; ++l) {
 #pragma unroll
-        for (int k = 0; k < PX; ++k) dpie_term<GRAD, HESS>(P.table[l], X[k], Y, acc[k], tb);
+        for (int k = 0; k < PX; ++k) dpie_term<GRAD, HESS>(P.table[l], X[k], Yk[k], acc[k], tb);
     }
     for (int l = e0; l < e1; ++l) {
 #pragma unroll
-        for (int k = 0; k < PX; ++k) nsie_term<GRAD, HESS>(P.table[l], X[k], Y, acc[k], tb);
+        for (int k = 0; k < PX; ++k) nsie_term<GRAD, HESS>(P.table[l], X[k], Yk[k], acc[k], tb);
     }
     for (int l = e1; l < e2; ++l) {
 #pragma unroll
-        for (int k = 0; k < PX; ++k) sis_term<GRAD, HESS>(P.table[l], X[k], Y, acc[k]);
+        for (int k = 0; k < PX; ++k) sis_term<GRAD, HESS>(P.table[l], X[k], Yk[k], acc[k]);
     }
     if (EXTREME) {
         const int e3 = b + P.cls_end[m][3];
         for (int l = e2; l < e3; ++l) {
 #pragma unroll
-            for (int k = 0; k < PX; ++k) extreme_term<GRAD, HESS>(P.table[l], X[k], Y, acc[k]);
+            for (int k = 0; k < PX; ++k) extreme_term<GRAD, HESS>(P.table[l], X[k], Yk[k], acc[k]);
         }
     }
     if (!inside) return;
@@ -372,7 +383,10 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
 
 template <bool GRAD, bool HESS, bool EXTREME>
 static cudaError_t launch_one(const LaunchParams &P, dim3 grid, cudaStream_t stream) {
-    superpose_kernel<GRAD, HESS, EXTREME><<<grid, dim3(THREADS, 1, 1), 0, stream>>>(P);
+    if (P.px)
+        superpose_kernel<GRAD, HESS, EXTREME, true><<<grid, dim3(THREADS, 1, 1), 0, stream>>>(P);
+    else
+        superpose_kernel<GRAD, HESS, EXTREME, false><<<grid, dim3(THREADS, 1, 1), 0, stream>>>(P);
     return cudaGetLastError();
 }
 
@@ -388,6 +402,7 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     Q.j0 = J.j0;
     for (int k = 0; k < 9; ++k) { Q.out[k] = J.out[k]; Q.m2[k] = J.stats ? J.m2[k] : nullptr; }
     Q.stats = 0;
+    Q.px = J.px; Q.py = J.py;
     Q.carry = J.carry;
     Q.math = J.math;
     Q.tiles_x = (J.nx + TILE_W - 1) / TILE_W;

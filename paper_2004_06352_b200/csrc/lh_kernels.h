@@ -26,6 +26,7 @@ struct LaunchParams {
     int stats;               // 0: out[] are per-model planes.  1 / 2: out[] are running MEANS over models and m2[] the
                              // running sums of squared deviations (Welford); 2 = last model: m2[] is divided by the count
     double *m2[9];           // stats only; nullptr = variance of that plane not wanted
+    const double *px, *py;   // POINTS variants only: coordinates of "pixel" i (then ny = 1, nx = number of points)
     unsigned short cls_end[LAUNCH_MODELS][CLS_COUNT];  // per model: end of each class, relative to its slice
     LensK table[LAUNCH_RECORDS];
 };
@@ -46,6 +47,7 @@ struct EvalJob {
     int nx, ny;      // ny = rows evaluated by this job
     int j0;          // first grid row (row slab of a larger grid; out[] / carry already point at that row)
     long long plane; // doubles between consecutive models / accumulators (the FULL plane, >= nx*ny)
+    const double *px, *py;  // DEVICE, both or neither: evaluate at these nx points (ny = 1) instead of the grid
     double *out[9];  // DEVICE
     double *m2[9];   // DEVICE, stats only (else all nullptr)
     int stats;       // 0 = per-model planes [nmodel][ny][nx]; 1 = mean / variance over the models, planes [ny][nx]

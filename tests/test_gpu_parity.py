@@ -239,6 +239,32 @@ def test_far_field_and_large_scales():
     check_planes(run_gpu(L, g, li.ALL_PLANES), ref_grid(L, g, li.ALL_PLANES), "far field")
 
 
+# ------------------------------------------------------------------ arbitrary points
+@pytest.mark.parametrize("npts", [1, 5, 127, 128, 129, 1000])
+def test_points_eval_matches_oracle_points(npts):
+    c = li.config(2)  # 500 mixed lenses: four lens chunks
+    rng = np.random.default_rng(npts)
+    xs, ys = rng.uniform(-90, 90, npts), rng.uniform(-90, 90, npts)
+    dx_, dy_ = torch.as_tensor(xs, device="cuda"), torch.as_tensor(ys, device="cuda")
+    out = dev_planes(li.ALL_PLANES, (npts,))
+    lh.lh_points_eval(c.lenses, dx_, dy_, **out)
+    torch.cuda.synchronize()
+    ref = oracle.points(c.lenses, xs, ys, planes=li.ALL_PLANES)
+    check_planes({n: v.cpu().numpy() for n, v in out.items()}, ref, f"{npts} points")
+
+
+def test_points_on_the_grid_equal_the_grid_call_bitwise():
+    c = li.config(1, scale=16)
+    g = c.grid
+    full = run_gpu(c.lenses, g, ("ax", "ay"))
+    X, Y = np.meshgrid(g.xs(), g.ys())
+    out = dev_planes(("ax", "ay"), (g.npix,))
+    lh.lh_points_eval(c.lenses, torch.as_tensor(X.ravel(), device="cuda"), torch.as_tensor(Y.ravel(), device="cuda"), **out)
+    torch.cuda.synchronize()
+    for n in full:
+        assert np.array_equal(out[n].cpu().numpy().reshape(g.ny, g.nx), full[n])
+
+
 # ------------------------------------------------------------------ multi-GPU primitive: row slabs
 @pytest.mark.parametrize("world", [2, 3, 8])
 def test_row_slabs_reassemble_the_full_map_bitwise(world):

@@ -33,7 +33,7 @@ def sass():
     return funcs
 
 
-FAST = ["ILb1ELb1ELb0", "ILb1ELb0ELb0", "ILb0ELb1ELb0"]  # <GRAD, HESS, EXTREME = false>
+FAST = ["ILb1ELb1ELb0ELb0E", "ILb1ELb0ELb0ELb0E", "ILb0ELb1ELb0ELb0E"]  # <GRAD, HESS, EXTREME = false, POINTS = false>
 
 
 @pytest.mark.parametrize("variant", FAST)
@@ -69,5 +69,5 @@ def test_no_spills_and_no_calls_in_fast_variants(sass, variant):
 
 
 def test_extreme_variants_exist_and_use_libdevice_paths(sass):
-    names = [n for n in sass if "superpose_kernel" in n and n.endswith("ELb1EEEvNS_12LaunchParamsE")]
-    assert len(names) == 3
+    names = [n for n in sass if "superpose_kernel" in n and re.search(r"ILb[01]ELb[01]ELb1ELb[01]E", n)]
+    assert len(names) == 6  # grad / hess / both, grid and points
