@@ -216,3 +216,17 @@ def model_slab(nmodel: int, rank: int, world: int):
     base, extra = divmod(nmodel, world)
     m0 = rank * base + min(rank, extra)
     return m0, m0 + base + (1 if rank < extra else 0)
+
+
+# ---------------------------------------------------------------- constraints (NEXT row f3)
+# 32-byte record == `lh_constraint` in include/lh.h (and the oracle's own declaration)
+CONSTRAINT_DTYPE = np.dtype([("source", "<i4"), ("_pad", "<i4"), ("x", "<f8"), ("y", "<f8"), ("sigma", "<f8")])
+
+
+def make_constraints(rows) -> np.ndarray:
+    """rows: iterable of (source, x, y, sigma)."""
+    rows = list(rows)
+    c = np.zeros(len(rows), dtype=CONSTRAINT_DTYPE)
+    for k, (s, x, y, sg) in enumerate(rows):
+        c[k] = (s, 0, x, y, sg)
+    return c

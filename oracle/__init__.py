@@ -199,3 +199,26 @@ def delens(ax, ay, x0: float, y0: float, dx: float, sources, max_images: int = 1
     found = L.orc_delens(ax.ctypes.data, ay.ctypes.data, x0, y0, dx, nx, ny, src.ctypes.data, len(src),
                          images.ctypes.data, max_images)
     return images[: min(found, max_images)], int(found)
+
+
+# ---------------------------------------------------------------- NEXT row f3: chi^2 of image constraints
+ORC_CONSTRAINT_DTYPE = np.dtype([("source", "<i4"), ("pad_", "<i4"), ("x", "<f8"), ("y", "<f8"), ("sigma", "<f8")])
+
+
+def chi2(lenses, x0: float, y0: float, dx: float, nx: int, ny: int, constraints, nsources: int) -> dict:
+    """PAPER.md:76-81 eq. 6 through the four stages of sec. 4.2 (readings R23): returns chi2, sources [N, 2],
+    predicted [K, 2] (the back-and-forth lensed constraint x_k), nimages."""
+    a = _as_lenses(lenses)
+    c = np.ascontiguousarray(constraints)
+    assert c.dtype.itemsize == 32
+    K = len(c)
+    src = np.empty((max(nsources, 1), 2), dtype=np.float64)
+    pred = np.empty((max(K, 1), 2), dtype=np.float64)
+    nim = C.c_longlong(0)
+    L = lib()
+    L.orc_chi2.restype = C.c_double
+    L.orc_chi2.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_int,
+                           C.c_int, C.c_void_p, C.c_void_p, C.POINTER(C.c_longlong)]
+    v = L.orc_chi2(a.ctypes.data, len(a), x0, y0, dx, nx, ny, c.ctypes.data, K, nsources, src.ctypes.data,
+                   pred.ctypes.data, C.byref(nim))
+    return {"chi2": float(v), "sources": src[:nsources], "predicted": pred[:K], "nimages": int(nim.value)}

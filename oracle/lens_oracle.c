@@ -301,3 +301,86 @@ long long orc_delens(const double *ax, const double *ay, double x0, double y0, d
         }
     return found;
 }
+
+/*
+ * ---- NEXT row f3: chi^2 of multiple-image constraints ---------------------------------------
+ * "Each image is unlensed onto the source-plane using the mass-model to be tested ... Sending back the
+ * barycentre of these positions to the image plane (see Fig. 3), we can define a cost-function
+ *   chi^2 = sum_i sum_j (c_ij - x_ij)^2 / sigma_ij^2"                  PAPER.md:76-81 (Fig. 3, eq. 6)
+ * Four stages (sec. 4.2): gradient on the grid; sources from the constraints; images
+ * by delensing and checking the grid; "the master CPU assigns them to their closest constraint and then
+ * computes the chi^2".  Readings R23, the paper being silent on each:
+ *   - beta_k = c_k - alpha(c_k) with alpha evaluated AT the constraint (not interpolated on the grid);
+ *   - source i = arithmetic mean of the beta_k of its constraints (Fig. 3 "barycentre"); a source
+ *     without constraints is ignored;
+ *   - predicted images of all sources by orc_delens on the grid;
+ *   - x_k = the predicted image of source s_k closest to c_k (so every constraint gets its closest
+ *     image; an image may serve several constraints or none);
+ *   - a constraint whose source has no predicted image on the grid contributes +infinity;
+ *   - (c - x)^2 is the squared Euclidean distance; the sum runs over the constraints in index order.
+ */
+#include <stdlib.h>
+
+typedef struct {
+    int32_t source; /* 0 .. nsources-1 */
+    int32_t pad_;
+    double x, y;    /* observed image position c_k */
+    double sigma;   /* > 0 */
+} orc_constraint;
+
+/* returns chi^2; sources_out [nsources][2] and predicted [K][2] may be NULL; *nimages = images found */
+double orc_chi2(const orc_lens *lenses, int nlens, double x0, double y0, double dx, int nx, int ny,
+                const orc_constraint *c, int K, int nsources, double *sources_out, double *predicted,
+                long long *nimages) {
+    double *src = (double *)calloc((size_t)(nsources > 0 ? nsources : 1) * 2, sizeof(double));
+    int *cnt = (int *)calloc((size_t)(nsources > 0 ? nsources : 1), sizeof(int));
+    /* stage 2: unlens the constraints, barycentre per source */
+    for (int k = 0; k < K; ++k) {
+        orc_deriv d;
+        orc_point(lenses, nlens, c[k].x, c[k].y, &d);
+        src[2 * c[k].source] += c[k].x - d.ax;
+        src[2 * c[k].source + 1] += c[k].y - d.ay;
+        cnt[c[k].source] += 1;
+    }
+    for (int i = 0; i < nsources; ++i) {
+        if (cnt[i] > 0) {
+            src[2 * i] /= (double)cnt[i];
+            src[2 * i + 1] /= (double)cnt[i];
+        } else {
+            src[2 * i] = src[2 * i + 1] = NAN; /* never inside a triangle */
+        }
+    }
+    /* stage 1: deflection on the grid */
+    const size_t np = (size_t)nx * (size_t)ny;
+    double *ax = (double *)malloc(np * sizeof(double)), *ay = (double *)malloc(np * sizeof(double));
+    orc_planes pl = {ax, ay, NULL, NULL, NULL, NULL, NULL, NULL, NULL};
+    orc_grid_rows(lenses, nlens, x0, y0, dx, nx, ny, 0, ny, &pl);
+    /* stage 3: predicted images */
+    long long cap = 64;
+    orc_image *im = (orc_image *)malloc((size_t)cap * sizeof(orc_image));
+    long long found = orc_delens(ax, ay, x0, y0, dx, nx, ny, src, nsources, im, cap);
+    if (found > cap) {
+        cap = found;
+        free(im);
+        im = (orc_image *)malloc((size_t)cap * sizeof(orc_image));
+        found = orc_delens(ax, ay, x0, y0, dx, nx, ny, src, nsources, im, cap);
+    }
+    /* stage 4: closest image of the same source, chi^2 */
+    double chi2 = 0.0;
+    for (int k = 0; k < K; ++k) {
+        double best = INFINITY, bx = NAN, by = NAN;
+        for (long long m = 0; m < found; ++m) {
+            if (im[m].source != c[k].source) continue;
+            const double ex = c[k].x - im[m].x, ey = c[k].y - im[m].y;
+            const double d2 = ex * ex + ey * ey;
+            if (d2 < best) { best = d2; bx = im[m].x; by = im[m].y; }
+        }
+        if (predicted) { predicted[2 * k] = bx; predicted[2 * k + 1] = by; }
+        chi2 += best / (c[k].sigma * c[k].sigma);
+    }
+    if (sources_out)
+        for (int i = 0; i < 2 * nsources; ++i) sources_out[i] = src[i];
+    if (nimages) *nimages = found;
+    free(im); free(ax); free(ay); free(cnt); free(src);
+    return chi2;
+}
