@@ -178,6 +178,32 @@ typedef struct {
 int lh_delens_grid(const double *ax, const double *ay, const lh_grid *g, const double *sources, int nsources,
                    lh_image *images, long long max_images, long long *count);
 
+/* ---- NEXT row f3: chi^2 of multiple-image constraints ------------------------------------------------------
+ * One observed image c_k of source `source`, with its positional error sigma. */
+typedef struct {
+    int32_t source; /* 0 .. nsources-1 */
+    int32_t _pad;
+    double x, y;    /* observed position c_k */
+    double sigma;   /* > 0 */
+} lh_constraint;
+
+/* chi^2 = sum_k |c_k - x_k|^2 / sigma_k^2 (eq. 6) through the four stages of PAPER.md:192-194, all on
+ * the device: (1) deflection on the grid; (2) every constraint unlensed at its own position, beta_k = c_k -
+ * alpha(c_k), source i = barycentre of its beta_k (Fig. 3); (3) predicted images of the sources by delensing the
+ * grid (lh_delens_grid); (4) x_k = the predicted image of c_k's source closest to c_k, summed in index order.
+ * A constraint whose source has no predicted image on the grid contributes +inf; a source without constraints is
+ * ignored (readings R23).
+ *   constraints  HOST [nconstraints], read during the call
+ *   chi2         DEVICE double[1]
+ *   predicted    DEVICE [nconstraints][2] or NULL: the x_k (NaN where there is none)
+ *   sources      DEVICE [nsources][2] or NULL: the barycentres (NaN for a source without constraints)
+ *   nimages      DEVICE long long[1] or NULL: predicted images found.  The library holds up to
+ *                64*nconstraints + 4096 of them; beyond that chi2 is NaN.
+ * Asynchronous on the set stream.  LH_EINVAL: as lh_grid_gradient, plus source index outside [0, nsources),
+ * sigma <= 0 or non-finite constraint. */
+int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constraint *constraints, int nconstraints,
+            int nsources, double *chi2, double *predicted, double *sources, long long *nimages);
+
 /* Same as lh_grid_eval_batch with HOST output planes: the library allocates (and
  * caches) device planes, runs the same kernel, copies the requested planes back
  * and synchronises the stream before returning.  Large jobs are cut into up to 8

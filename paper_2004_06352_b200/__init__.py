@@ -69,6 +69,8 @@ def _load():
         L.lh_grid_eval_host.argtypes = [vp, ci, ci, gp, op]
         L.lh_grid_stats_batch.argtypes = [vp, ci, ci, gp, op, op]
         L.lh_grid_stats_batch.restype = ci
+        L.lh_chi2.argtypes = [vp, ci, gp, vp, ci, ci, dp, dp, dp, vp]
+        L.lh_chi2.restype = ci
         L.lh_points_eval.argtypes = [vp, ci, dp, dp, C.c_longlong, op]
         L.lh_points_eval.restype = ci
         L.lh_grid_eval_rows.argtypes = [vp, ci, gp, ci, ci, op]
@@ -167,6 +169,17 @@ def lh_grid_eval(lenses, grid, **planes):
     a, p, n = _lenses_ptr(lenses)
     o = _outputs(planes, _dev_ptr)
     _check(_load().lh_grid_eval(p, n, C.byref(_grid(grid)), C.byref(o)))
+
+
+def lh_chi2(lenses, grid, constraints, nsources: int, chi2, predicted=None, sources=None, nimages=None):
+    """constraints: host array of 32-byte lh_constraint records (lens_inputs.CONSTRAINT_DTYPE); chi2: device float64[1];
+    predicted [K, 2], sources [nsources, 2]: device float64 or None; nimages: device int64[1] or None."""
+    a, p, n = _lenses_ptr(lenses)
+    c = np.ascontiguousarray(constraints)
+    if c.dtype.itemsize != 32:
+        raise TypeError("constraints must be an array of 32-byte lh_constraint records")
+    _check(_load().lh_chi2(p, n, C.byref(_grid(grid)), c.ctypes.data, c.size, int(nsources), _dev_ptr(chi2),
+                           _dev_ptr(predicted), _dev_ptr(sources), None if nimages is None else nimages.data_ptr()))
 
 
 def lh_points_eval(lenses, xs, ys, **planes):

@@ -17,6 +17,15 @@ namespace lh {
 cudaError_t launch_delens(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,
                           const double *sources, int ns, lh_image *images, long long max_images,
                           unsigned long long *count, int sms, cudaStream_t st, long long *launches);
+cudaError_t launch_delens_dev(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,
+                              const double *dsources, int ns, lh_image *images, long long max_images,
+                              unsigned long long *count, int sms, cudaStream_t st, long long *launches);
+cudaError_t launch_constraint_points(const lh_constraint *c, int K, double *cx, double *cy, cudaStream_t st);
+cudaError_t launch_barycentre(const lh_constraint *c, int K, const double *ax, const double *ay, int nsources, double *src,
+                              cudaStream_t st);
+cudaError_t launch_assign_and_sum(const lh_constraint *c, int K, const lh_image *im, const unsigned long long *count,
+                                  long long cap, double *pred, double *term, double *chi2, long long *nimages,
+                                  cudaStream_t st);
 }
 
 namespace {
@@ -50,6 +59,8 @@ struct Context {
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_piece[PIECES] = {};
     double *d_sink = nullptr;
+    char *d_chi = nullptr;  // scratch of lh_chi2 (deflection planes, constraint arrays, sources, images)
+    size_t chi_bytes = 0;
 
     ~Context() {
         // process teardown: the CUDA runtime may already be gone; leak deliberately.
@@ -419,6 +430,92 @@ int lh_delens_grid(const double *ax, const double *ay, const lh_grid *g, const d
     CU(cudaMemsetAsync(count, 0, sizeof(long long), ctx.stream));
     CU(lh::launch_delens(ax, ay, g->x0, g->y0, g->dx, g->nx, g->ny, sources, nsources, images, max_images,
                          reinterpret_cast<unsigned long long *>(count), sms, ctx.stream, &ctx.launches));
+    return LH_OK;
+}
+
+int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constraint *constraints, int nconstraints,
+            int nsources, double *chi2, double *predicted, double *sources, long long *nimages) {
+    ctx.err[0] = 0;
+    int rc = check_common(lenses, 1, nlens, g);
+    if (rc) return rc;
+    const int K = nconstraints, N = nsources;
+    if (K < 0 || N < 0 || (K > 0 && !constraints)) return fail(LH_EINVAL, "lh_chi2: bad constraint list");
+    if (!chi2) return fail(LH_EINVAL, "lh_chi2: chi2 is required");
+    for (int k = 0; k < K; ++k) {
+        const lh_constraint &c = constraints[k];
+        if (c.source < 0 || c.source >= N) return fail(LH_EINVAL, "constraint %d: source index outside [0, nsources)", k);
+        if (!(std::isfinite(c.x) && std::isfinite(c.y) && std::isfinite(c.sigma)) || !(c.sigma > 0.0))
+            return fail(LH_EINVAL, "constraint %d: non-finite position or sigma <= 0", k);
+    }
+    if ((rc = check_device_ptr(chi2, "chi2"))) return rc;
+    if (predicted && (rc = check_device_ptr(predicted, "predicted"))) return rc;
+    if (sources && (rc = check_device_ptr(sources, "sources"))) return rc;
+    if (nimages && (rc = check_device_ptr(reinterpret_cast<double *>(nimages), "nimages"))) return rc;
+    {  // validate the lens list before anything is enqueued
+        lh::ModelRanges r;
+        try {
+            ctx.h_table.resize((size_t)nlens);
+        } catch (const std::bad_alloc &) {
+            return fail(LH_EINVAL, "out of host memory packing %d lenses", nlens);
+        }
+        if (lh::pack_model(lenses, nlens, ctx.h_table.data(), &r, ctx.err, sizeof(ctx.err), 0) != 0) return LH_EINVAL;
+    }
+
+    // scratch layout (all 16-byte aligned)
+    const size_t npix = (size_t)g->nx * g->ny;
+    const long long cap = 64LL * K + 4096;
+    auto al = [](size_t b) { return (b + 15) & ~size_t(15); };
+    const size_t o_ax = 0, o_ay = o_ax + al(npix * 8), o_c = o_ay + al(npix * 8), o_cx = o_c + al((size_t)K * 32 + 16),
+                 o_cy = o_cx + al((size_t)K * 8 + 16), o_bax = o_cy + al((size_t)K * 8 + 16),
+                 o_bay = o_bax + al((size_t)K * 8 + 16), o_term = o_bay + al((size_t)K * 8 + 16),
+                 o_src = o_term + al((size_t)K * 8 + 16), o_cnt = o_src + al((size_t)N * 16 + 16), o_im = o_cnt + 16,
+                 total = o_im + (size_t)cap * sizeof(lh_image);
+    if (total > ctx.chi_bytes) {
+        if (ctx.d_chi) {
+            CU(cudaStreamSynchronize(ctx.stream));
+            cudaFree(ctx.d_chi);
+            ctx.d_chi = nullptr;
+            ctx.chi_bytes = 0;
+        }
+        CU(cudaMalloc(&ctx.d_chi, total));
+        ctx.chi_bytes = total;
+    }
+    char *B = ctx.d_chi;
+    double *ax = reinterpret_cast<double *>(B + o_ax), *ay = reinterpret_cast<double *>(B + o_ay);
+    lh_constraint *dc = reinterpret_cast<lh_constraint *>(B + o_c);
+    double *cx = reinterpret_cast<double *>(B + o_cx), *cy = reinterpret_cast<double *>(B + o_cy);
+    double *bax = reinterpret_cast<double *>(B + o_bax), *bay = reinterpret_cast<double *>(B + o_bay);
+    double *term = reinterpret_cast<double *>(B + o_term);
+    double *src = sources ? sources : reinterpret_cast<double *>(B + o_src);
+    unsigned long long *cnt = reinterpret_cast<unsigned long long *>(B + o_cnt);
+    lh_image *im = reinterpret_cast<lh_image *>(B + o_im);
+    cudaStream_t s = ctx.stream;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+
+    // stage 2: unlens the constraints at their own positions, barycentre per source
+    if (K > 0) {
+        CU(cudaMemcpyAsync(dc, constraints, (size_t)K * sizeof(lh_constraint), cudaMemcpyHostToDevice, s));
+        CU(lh::launch_constraint_points(dc, K, cx, cy, s));
+        ++ctx.launches;
+        lh_grid pg = {0.0, 0.0, 1.0, K, 1};
+        double *po[NPLANES] = {bax, bay, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+        EvalOpts opt;
+        opt.px = cx; opt.py = cy;
+        if ((rc = eval_device(lenses, 1, nlens, &pg, po, opt))) return rc;
+    }
+    CU(lh::launch_barycentre(dc, K, bax, bay, N, src, s));
+    ++ctx.launches;
+    // stage 1: deflection on the grid
+    double *go[NPLANES] = {ax, ay, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    if ((rc = eval_device(lenses, 1, nlens, g, go))) return rc;
+    // stage 3: predicted images
+    CU(cudaMemsetAsync(cnt, 0, sizeof(*cnt), s));
+    CU(lh::launch_delens_dev(ax, ay, g->x0, g->y0, g->dx, g->nx, g->ny, src, N, im, cap, cnt, sms, s, &ctx.launches));
+    // stage 4: closest image of the same source, chi^2
+    CU(lh::launch_assign_and_sum(dc, K, im, cnt, cap, predicted, term, chi2, nimages, s));
+    ctx.launches += (K > 0) + 1;
     return LH_OK;
 }
 

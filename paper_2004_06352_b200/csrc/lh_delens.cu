@@ -34,6 +34,7 @@ struct DelensParams {
     double x0, y0, dx;
     int nx, ny;
     int source0, nsources;  // global index of src[0]; sources in this launch
+    const double *dsrc;     // DEV_SRC variant: DEVICE [nsources][2] (f3: sources computed on the device); else nullptr
     double src[DELENS_SOURCES][2];
 };
 static_assert(sizeof(DelensParams) <= 32764, "kernel parameter space");
@@ -63,6 +64,7 @@ __device__ __forceinline__ void test_triangle(const DelensParams &P, int s, doub
     P.images[k] = im;
 }
 
+template <bool DEV_SRC>
 __global__ void __launch_bounds__(DELENS_THREADS) delens_kernel(const __grid_constant__ DelensParams P) {
     const long long ncx = P.nx - 1, ncells = ncx * (P.ny - 1);
     for (long long cell = (long long)blockIdx.x * DELENS_THREADS + threadIdx.x; cell < ncells;
@@ -82,7 +84,8 @@ __global__ void __launch_bounds__(DELENS_THREADS) delens_kernel(const __grid_con
             loy = fmin(loy, B[c][1]); hiy = fmax(hiy, B[c][1]);
         }
         for (int s = 0; s < P.nsources; ++s) {
-            const double sx = P.src[s][0], sy = P.src[s][1];
+            const double sx = DEV_SRC ? __ldg(P.dsrc + 2 * s) : P.src[s][0];
+            const double sy = DEV_SRC ? __ldg(P.dsrc + 2 * s + 1) : P.src[s][1];
             // a point of a closed triangle lies inside the bounding box of its vertices: exact reject
             if (sx < lox || sx > hix || sy < loy || sy > hiy) continue;
             test_triangle(P, s, sx, sy, T, B, 0, 1, 2, 2 * cell);
@@ -126,12 +129,97 @@ cudaError_t launch_delens(const double *ax, const double *ay, double x0, double 
         const int n = ns - s0 < DELENS_SOURCES ? ns - s0 : DELENS_SOURCES;
         P.source0 = s0; P.nsources = n;
         for (int s = 0; s < n; ++s) { P.src[s][0] = sources[2 * (s0 + s)]; P.src[s][1] = sources[2 * (s0 + s) + 1]; }
-        delens_kernel<<<(unsigned)blocks, DELENS_THREADS, 0, st>>>(P);
+        P.dsrc = nullptr;
+        delens_kernel<false><<<(unsigned)blocks, DELENS_THREADS, 0, st>>>(P);
         ++*launches;
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
+}
+
+// sources: DEVICE [ns][2] (a NaN source matches nothing).  One launch; `count` must be zero on entry.
+cudaError_t launch_delens_dev(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,
+                              const double *dsources, int ns, lh_image *images, long long max_images,
+                              unsigned long long *count, int sms, cudaStream_t st, long long *launches) {
+    thread_local DelensParams P;
+    P.ax = ax; P.ay = ay; P.images = images; P.count = count; P.max_images = max_images;
+    P.x0 = x0; P.y0 = y0; P.dx = dx; P.nx = nx; P.ny = ny;
+    P.source0 = 0; P.nsources = ns; P.dsrc = dsources;
+    const long long ncells = (long long)(nx - 1) * (ny - 1);
+    if (ncells <= 0 || ns <= 0) return cudaSuccess;
+    long long blocks = (ncells + DELENS_THREADS - 1) / DELENS_THREADS;
+    if (blocks > (long long)sms * 8) blocks = (long long)sms * 8;
+    delens_kernel<true><<<(unsigned)blocks, DELENS_THREADS, 0, st>>>(P);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+// ---- f3: the small stages of the chi^2 pipeline (PAPER.md:76-81 eq. 6, :192-194; readings R23) -------------
+__global__ void constraint_points_kernel(const lh_constraint *c, int K, double *cx, double *cy) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < K) { cx[k] = c[k].x; cy[k] = c[k].y; }
+}
+
+// stage 2: source i = barycentre of beta_k = c_k - alpha(c_k) over its constraints, summed in index order
+__global__ void barycentre_kernel(const lh_constraint *c, int K, const double *ax, const double *ay, int nsources,
+                                  double *src) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nsources) return;
+    double sx = 0.0, sy = 0.0;
+    int n = 0;
+    for (int k = 0; k < K; ++k) {
+        if (c[k].source != i) continue;
+        sx = __dadd_rn(sx, __dsub_rn(c[k].x, ax[k]));
+        sy = __dadd_rn(sy, __dsub_rn(c[k].y, ay[k]));
+        ++n;
+    }
+    src[2 * i] = n ? __ddiv_rn(sx, (double)n) : NAN;
+    src[2 * i + 1] = n ? __ddiv_rn(sy, (double)n) : NAN;
+}
+
+// stage 4a: x_k = predicted image of the constraint's source closest to it; term_k = |c_k - x_k|^2 / sigma_k^2
+__global__ void assign_kernel(const lh_constraint *c, int K, const lh_image *im, const unsigned long long *count,
+                              long long cap, double *pred, double *term) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= K) return;
+    const long long n = *count < (unsigned long long)cap ? (long long)*count : cap;
+    double best = INFINITY, bx = NAN, by = NAN;
+    for (long long m = 0; m < n; ++m) {
+        if (im[m].source != c[k].source) continue;
+        const double ex = __dsub_rn(c[k].x, im[m].x), ey = __dsub_rn(c[k].y, im[m].y);
+        const double d2 = __dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey));
+        if (d2 < best) { best = d2; bx = im[m].x; by = im[m].y; }
+    }
+    if (pred) { pred[2 * k] = bx; pred[2 * k + 1] = by; }
+    term[k] = __ddiv_rn(best, __dmul_rn(c[k].sigma, c[k].sigma));
+}
+
+// stage 4b: chi^2 = sum of the terms in index order (one thread: K is a few hundred; the order is the definition's).
+// More images than the buffer holds -> NaN (the assignment above did not see them all).
+__global__ void chi2_sum_kernel(const double *term, int K, const unsigned long long *count, long long cap, double *chi2,
+                                long long *nimages) {
+    double s = 0.0;
+    for (int k = 0; k < K; ++k) s = __dadd_rn(s, term[k]);
+    *chi2 = (*count > (unsigned long long)cap) ? NAN : s;
+    if (nimages) *nimages = (long long)*count;
+}
+
+cudaError_t launch_constraint_points(const lh_constraint *c, int K, double *cx, double *cy, cudaStream_t st) {
+    if (K > 0) constraint_points_kernel<<<(K + 127) / 128, 128, 0, st>>>(c, K, cx, cy);
+    return cudaGetLastError();
+}
+cudaError_t launch_barycentre(const lh_constraint *c, int K, const double *ax, const double *ay, int nsources, double *src,
+                              cudaStream_t st) {
+    if (nsources > 0) barycentre_kernel<<<(nsources + 127) / 128, 128, 0, st>>>(c, K, ax, ay, nsources, src);
+    return cudaGetLastError();
+}
+cudaError_t launch_assign_and_sum(const lh_constraint *c, int K, const lh_image *im, const unsigned long long *count,
+                                  long long cap, double *pred, double *term, double *chi2, long long *nimages,
+                                  cudaStream_t st) {
+    if (K > 0) assign_kernel<<<(K + 127) / 128, 128, 0, st>>>(c, K, im, count, cap, pred, term);
+    chi2_sum_kernel<<<1, 1, 0, st>>>(term, K, count, cap, chi2, nimages);
+    return cudaGetLastError();
 }
 
 }  // namespace lh
