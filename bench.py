@@ -67,6 +67,9 @@ def parse():
     ap.add_argument("--delens", action="store_true",
                     help="NEXT row f1 alone (not the default bench line): lh_delens_grid on the deflection planes of "
                          "--config (default 3) for 80 synthetic sources (M1149 has 80, PAPER.md:208)")
+    ap.add_argument("--chi2", action="store_true",
+                    help="NEXT row f3 alone (not the default bench line): lh_chi2 on --config (default 3) with 80 "
+                         "sources / 227 image constraints (the shape of M1149, PAPER.md:208) at seeded random positions")
     ap.add_argument("--stats", action="store_true",
                     help="NEXT row f2 on a batch config (use --config 4): per-pixel mean and variance of ax ay kappa "
                          "gamma1 gamma2 over the models through lh_grid_stats_batch (not the default bench line)")
@@ -332,6 +335,48 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_chi2(args):
+    """f3 measured alone: one step = one chi^2 evaluation (all four stages of PAPER.md:192-194 on the device)."""
+    import torch
+
+    import paper_2004_06352_b200 as lh
+
+    torch.cuda.set_device(0)
+    cfg = li.config(args.config)
+    g, L = cfg.grid, cfg.lenses[: cfg.nlens]
+    rng = np.random.default_rng(1)
+    ns, K = 80, 227
+    half = 0.3 * g.nx * g.dx / 2
+    cons = li.make_constraints((k if k < ns else int(rng.integers(0, ns)), rng.uniform(-half, half),
+                                rng.uniform(-half, half), 0.3) for k in range(K))
+    chi = torch.zeros(1, dtype=torch.float64, device="cuda")
+    nim = torch.zeros(1, dtype=torch.int64, device="cuda")
+    stream = torch.cuda.current_stream()
+    lh.lh_set_stream(stream)
+    for _ in range(max(args.warmup, 3)):
+        lh.lh_chi2(L, g, cons, ns, chi, None, None, nim)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    n0 = lh.lh_launch_count()
+    with ClockSampler(0) as clk:
+        for a, b in ev:
+            a.record(stream)
+            lh.lh_chi2(L, g, cons, ns, chi, None, None, nim)
+            b.record(stream)
+        torch.cuda.synchronize()
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    evals = g.npix * cfg.nlens + K * cfg.nlens
+    line = {"metric": "chi^2 evaluations/sec (eq. 6, four stages)", "value": 1e3 / ms, "unit": "chi2/s", "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "chi2": float(chi.item()), "images_found": int(nim.item()),
+            "gradient_evals_per_s": evals / (ms * 1e-3),
+            "config": {"workload": f"NEXT row f3: configs[{args.config}] {g.nx}x{g.ny} px x {cfg.nlens} lenses, "
+                                   f"{ns} sources, {K} image constraints"},
+            "clocks": clk.summary(), "gpu_launches": int(lh.lh_launch_count() - n0)}
+    print(json.dumps(line), flush=True)
+
+
 def run_delens(args):
     """f1 measured alone: one step = lh_delens_grid over the whole grid for 80 sources (deflection planes resident)."""
     import torch
@@ -395,6 +440,9 @@ def run_delens(args):
 
 if __name__ == "__main__":
     a = parse()
+    if a.chi2 and a.impl != "reference":
+        run_chi2(a)
+        raise SystemExit(0)
     if a.delens and a.impl != "reference":
         run_delens(a)
         raise SystemExit(0)
