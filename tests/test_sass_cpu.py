@@ -52,20 +52,26 @@ def test_no_spills_and_no_calls_in_fast_variants(sass, variant):
     name = next(n for n in sass if "superpose_kernel" in n and variant in n)
     body = "\n".join(sass[name])
     assert not re.search(r"\b(STL|LDL)\b", body), "local-memory traffic (register spill)"
-    # the only calls allowed are the IEEE-division slow paths of the per-pixel epilogue (mu = 1/det),
-    # which sit after the last lens loop
-    last_backedge, calls = -1, []
+    # the only calls allowed are the IEEE-division slow paths of the per-pixel epilogue (mu = 1/det): they may sit
+    # inside a loop that holds other loops (a persistent loop over pixel tiles) but in no lens loop
+    loops, calls = [], []
     for line in sass[name]:
         m = re.search(r"/\*([0-9a-f]{4,})\*/\s+(?:@!?U?P\d\s+)?(BRA(?:\.U)?|CALL\S*)\s+(?:!?U?P\d,\s+)?0x([0-9a-f]+)", line)
         if not m:
             continue
         at, op, to = int(m.group(1), 16), m.group(2), int(m.group(3), 16)
         if op.startswith("BRA") and to < at:
-            last_backedge = max(last_backedge, at)
+            loops.append((to, at))
         if op.startswith("CALL"):
             calls.append(at)
-    assert last_backedge > 0
-    assert all(c > last_backedge for c in calls), "a slow-path call inside a lens loop of a fast variant"
+    assert loops
+
+    def is_outer(l):  # a loop that holds other loops (e.g. a persistent loop over pixel tiles) is not a lens loop
+        return any(m != l and l[0] <= m[0] and m[1] <= l[1] for m in loops)
+
+    for c in calls:
+        inside = [l for l in loops if l[0] <= c <= l[1] and not is_outer(l)]
+        assert not inside, "a slow-path call inside a lens loop of a fast variant"
 
 
 def test_extreme_variants_exist_and_use_libdevice_paths(sass):
