@@ -39,14 +39,9 @@ using lh::ModelRanges;
 // rewritten as soon as launch_eval returns.  `d_carry` (accumulators handed from one lens
 // chunk of a model to the next) is reused across calls: stream order protects it on one
 // stream, ev_done + cudaStreamWaitEvent across a stream change.
-struct Context {
-    cudaStream_t stream = nullptr;
-    char err[512] = {0};
-    long long launches = 0;
-
-    std::vector<LensK> h_table, h_shared;
-    std::vector<ModelRanges> h_ranges;
-
+// Everything that lives on ONE device: cached buffers, events, the copy stream.  A host thread may switch
+// devices between calls (cudaSetDevice / torch.cuda.set_device); each device then gets its own state.
+struct DeviceState {
     double *d_carry = nullptr;
     size_t carry_bytes = 0;
     cudaEvent_t ev_done = nullptr;
@@ -61,6 +56,18 @@ struct Context {
     double *d_sink = nullptr;
     char *d_chi = nullptr;  // scratch of lh_chi2 (deflection planes, constraint arrays, sources, images)
     size_t chi_bytes = 0;
+};
+
+struct Context {
+    cudaStream_t stream = nullptr;
+    char err[512] = {0};
+    long long launches = 0;
+
+    std::vector<LensK> h_table, h_shared;
+    std::vector<ModelRanges> h_ranges;
+
+    static const int MAX_DEVICES = 64;
+    DeviceState dev[MAX_DEVICES];
 
     ~Context() {
         // process teardown: the CUDA runtime may already be gone; leak deliberately.
@@ -68,6 +75,13 @@ struct Context {
 };
 
 thread_local Context ctx;
+
+// state of the device that is current on this host thread
+DeviceState &DS() {
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= Context::MAX_DEVICES) d = 0;
+    return ctx.dev[d];
+}
 
 // The atan / atanh reduction tables (lh_math.cuh): one read-only device copy per device,
 // made on first use and kept for the life of the process.
@@ -176,18 +190,18 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     }
 
     cudaStream_t s = ctx.stream;
-    if (!ctx.ev_done) CU(cudaEventCreateWithFlags(&ctx.ev_done, cudaEventDisableTiming));
+    if (!DS().ev_done) CU(cudaEventCreateWithFlags(&DS().ev_done, cudaEventDisableTiming));
     const size_t carry_need =
         (nlens > lh::LAUNCH_RECORDS || nshared > 0) ? (size_t)5 * g->nx * g->ny * sizeof(double) : 0;
-    if (carry_need > ctx.carry_bytes) {
-        if (ctx.busy) CU(cudaEventSynchronize(ctx.ev_done));  // the old buffer is no longer in use
-        if (ctx.d_carry) cudaFree(ctx.d_carry);
-        ctx.d_carry = nullptr;
-        ctx.carry_bytes = 0;
-        CU(cudaMalloc(&ctx.d_carry, carry_need));
-        ctx.carry_bytes = carry_need;
+    if (carry_need > DS().carry_bytes) {
+        if (DS().busy) CU(cudaEventSynchronize(DS().ev_done));  // the old buffer is no longer in use
+        if (DS().d_carry) cudaFree(DS().d_carry);
+        DS().d_carry = nullptr;
+        DS().carry_bytes = 0;
+        CU(cudaMalloc(&DS().d_carry, carry_need));
+        DS().carry_bytes = carry_need;
     }
-    if (carry_need && ctx.busy && ctx.last_stream != s) CU(cudaStreamWaitEvent(s, ctx.ev_done, 0));
+    if (carry_need && DS().busy && DS().last_stream != s) CU(cudaStreamWaitEvent(s, DS().ev_done, 0));
 
     int dev = 0;
     CU(cudaGetDevice(&dev));
@@ -214,12 +228,12 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     J.stats = dev_m2 ? 1 : 0;
     // carry is laid out like the planes it serves: a slab of FULL-size planes (nrows < g->ny) uses the slab's rows
     // of a full-size carry; a stand-alone slab (lh_grid_eval_rows: g->ny == nrows) uses a carry of its own size
-    J.carry = ctx.d_carry ? ctx.d_carry + (nrows != g->ny ? (size_t)j0 * g->nx : 0) : nullptr;
+    J.carry = DS().d_carry ? DS().d_carry + (nrows != g->ny ? (size_t)j0 * g->nx : 0) : nullptr;
     CU(lh::launch_eval(J, s, &ctx.launches));
     if (carry_need) {
-        CU(cudaEventRecord(ctx.ev_done, s));
-        ctx.busy = true;
-        ctx.last_stream = s;
+        CU(cudaEventRecord(DS().ev_done, s));
+        DS().busy = true;
+        DS().last_stream = s;
     }
     return LH_OK;
 }
@@ -470,17 +484,17 @@ int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constra
                  o_bay = o_bax + al((size_t)K * 8 + 16), o_term = o_bay + al((size_t)K * 8 + 16),
                  o_src = o_term + al((size_t)K * 8 + 16), o_cnt = o_src + al((size_t)N * 16 + 16), o_im = o_cnt + 16,
                  total = o_im + (size_t)cap * sizeof(lh_image);
-    if (total > ctx.chi_bytes) {
-        if (ctx.d_chi) {
+    if (total > DS().chi_bytes) {
+        if (DS().d_chi) {
             CU(cudaStreamSynchronize(ctx.stream));
-            cudaFree(ctx.d_chi);
-            ctx.d_chi = nullptr;
-            ctx.chi_bytes = 0;
+            cudaFree(DS().d_chi);
+            DS().d_chi = nullptr;
+            DS().chi_bytes = 0;
         }
-        CU(cudaMalloc(&ctx.d_chi, total));
-        ctx.chi_bytes = total;
+        CU(cudaMalloc(&DS().d_chi, total));
+        DS().chi_bytes = total;
     }
-    char *B = ctx.d_chi;
+    char *B = DS().d_chi;
     double *ax = reinterpret_cast<double *>(B + o_ax), *ay = reinterpret_cast<double *>(B + o_ay);
     lh_constraint *dc = reinterpret_cast<lh_constraint *>(B + o_c);
     double *cx = reinterpret_cast<double *>(B + o_cx), *cy = reinterpret_cast<double *>(B + o_cy);
@@ -531,31 +545,31 @@ int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_gri
     if (!nreq) return fail(LH_EINVAL, "no output plane requested");
     const size_t plane_bytes = (size_t)nmodel * g->nx * g->ny * sizeof(double);
     const size_t need = plane_bytes * nreq;
-    if (need > ctx.planes_bytes) {
-        if (ctx.d_planes) {
+    if (need > DS().planes_bytes) {
+        if (DS().d_planes) {
             CU(cudaStreamSynchronize(ctx.stream));
-            cudaFree(ctx.d_planes);
-            ctx.d_planes = nullptr;
-            ctx.planes_bytes = 0;
+            cudaFree(DS().d_planes);
+            DS().d_planes = nullptr;
+            DS().planes_bytes = 0;
         }
-        CU(cudaMalloc(&ctx.d_planes, need));
-        ctx.planes_bytes = need;
+        CU(cudaMalloc(&DS().d_planes, need));
+        DS().planes_bytes = need;
     }
     int slot = 0;
     for (int k = 0; k < NPLANES; ++k)
-        dp[k] = hp[k] ? ctx.d_planes + (size_t)(slot++) * (plane_bytes / sizeof(double)) : nullptr;
+        dp[k] = hp[k] ? DS().d_planes + (size_t)(slot++) * (plane_bytes / sizeof(double)) : nullptr;
 
     // Pipeline: the work is cut into pieces (row slabs of one map, or groups of models of a batch); the
     // device-to-host copy of piece k runs on a second stream while piece k+1 is being computed.
-    if (!ctx.copy_stream) {
-        CU(cudaStreamCreateWithFlags(&ctx.copy_stream, cudaStreamNonBlocking));
-        for (int k = 0; k < Context::PIECES; ++k) CU(cudaEventCreateWithFlags(&ctx.ev_piece[k], cudaEventDisableTiming));
+    if (!DS().copy_stream) {
+        CU(cudaStreamCreateWithFlags(&DS().copy_stream, cudaStreamNonBlocking));
+        for (int k = 0; k < DeviceState::PIECES; ++k) CU(cudaEventCreateWithFlags(&DS().ev_piece[k], cudaEventDisableTiming));
     }
     const size_t npix = (size_t)g->nx * g->ny;
     const int units = nmodel == 1 ? g->ny : nmodel;  // rows or models
     // small jobs are not worth cutting: about 4 MB of results per piece at least
     long long want = (long long)(need >> 22);
-    const int pieces = want < 1 ? 1 : (want > Context::PIECES ? Context::PIECES : (int)want);
+    const int pieces = want < 1 ? 1 : (want > DeviceState::PIECES ? DeviceState::PIECES : (int)want);
     int per = (units + pieces - 1) / pieces;
     if (nmodel == 1) per = (per + 7) & ~7;            // whole pixel tiles
     int piece = 0;
@@ -570,15 +584,15 @@ int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_gri
         rc = nmodel == 1 ? eval_device(lenses, 1, nlens, g, sub, opt)
                          : eval_device(lenses + (size_t)u0 * nlens, nu, nlens, g, sub);
         if (rc) {
-            cudaStreamSynchronize(ctx.copy_stream);
+            cudaStreamSynchronize(DS().copy_stream);
             return rc;  // a lens was rejected on the first piece: nothing enqueued, nothing written
         }
-        CU(cudaEventRecord(ctx.ev_piece[piece], ctx.stream));
-        CU(cudaStreamWaitEvent(ctx.copy_stream, ctx.ev_piece[piece], 0));
+        CU(cudaEventRecord(DS().ev_piece[piece], ctx.stream));
+        CU(cudaStreamWaitEvent(DS().copy_stream, DS().ev_piece[piece], 0));
         for (int k = 0; k < NPLANES; ++k)
-            if (hp[k]) CU(cudaMemcpyAsync(hp[k] + off, dp[k] + off, count * sizeof(double), cudaMemcpyDeviceToHost, ctx.copy_stream));
+            if (hp[k]) CU(cudaMemcpyAsync(hp[k] + off, dp[k] + off, count * sizeof(double), cudaMemcpyDeviceToHost, DS().copy_stream));
     }
-    CU(cudaStreamSynchronize(ctx.copy_stream));
+    CU(cudaStreamSynchronize(DS().copy_stream));
     CU(cudaStreamSynchronize(ctx.stream));
     return LH_OK;
 }
@@ -613,14 +627,14 @@ int lh_fp64_peak_probe(int iters, double *flops_per_s, double *seconds) {
     int dev = 0, sms = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    if (!ctx.d_sink) CU(cudaMalloc(&ctx.d_sink, 64));
+    if (!DS().d_sink) CU(cudaMalloc(&DS().d_sink, 64));
     const int blocks = sms * 8;  // 8 x 256 threads = 64 warps per SM
     cudaEvent_t t0, t1;
     CU(cudaEventCreate(&t0));
     CU(cudaEventCreate(&t1));
-    CU(lh::launch_dfma_probe(iters / 8 + 1, blocks, ctx.d_sink, ctx.stream));  // warm-up
+    CU(lh::launch_dfma_probe(iters / 8 + 1, blocks, DS().d_sink, ctx.stream));  // warm-up
     CU(cudaEventRecord(t0, ctx.stream));
-    CU(lh::launch_dfma_probe(iters, blocks, ctx.d_sink, ctx.stream));
+    CU(lh::launch_dfma_probe(iters, blocks, DS().d_sink, ctx.stream));
     CU(cudaEventRecord(t1, ctx.stream));
     CU(cudaEventSynchronize(t1));
     ctx.launches += 2;
@@ -663,19 +677,19 @@ int lh_fp64_issue_probe(int variant, int extra, int warps_per_subpartition, int 
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     CU(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev));
-    if (!ctx.d_sink) CU(cudaMalloc(&ctx.d_sink, 64));
+    if (!DS().d_sink) CU(cudaMalloc(&DS().d_sink, 64));
     const int blocks = sms * warps_per_subpartition;  // 128 threads = one warp per sub-partition per block
     cudaEvent_t t0, t1;
     CU(cudaEventCreate(&t0));
     CU(cudaEventCreate(&t1));
-    cudaError_t e = lh::launch_issue_probe(variant, extra, iters / 8 + 1, blocks, ctx.d_sink, ctx.stream);  // warm-up
+    cudaError_t e = lh::launch_issue_probe(variant, extra, iters / 8 + 1, blocks, DS().d_sink, ctx.stream);  // warm-up
     if (e == cudaErrorInvalidValue) {
         cudaGetLastError();
         return fail(LH_EINVAL, "lh_fp64_issue_probe: unknown variant %d / extra %d", variant, extra);
     }
     CU(e);
     CU(cudaEventRecord(t0, ctx.stream));
-    CU(lh::launch_issue_probe(variant, extra, iters, blocks, ctx.d_sink, ctx.stream));
+    CU(lh::launch_issue_probe(variant, extra, iters, blocks, DS().d_sink, ctx.stream));
     CU(cudaEventRecord(t1, ctx.stream));
     CU(cudaEventSynchronize(t1));
     ctx.launches += 2;
