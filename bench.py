@@ -37,11 +37,11 @@ METRIC = "pixel-lens FP64 gradient+Hessian evals/sec"
 UNIT = "evals/s"
 
 # Executed FP64 flops per (pixel, lens) dPIE evaluation of each kernel variant (2*DFMA + DMUL + DADD
-# thread-instructions / evaluations).  grad+hess: ncu counters, profiles/r01_cfg3_ncu.md (83.0 FP64
-# instructions, 122.0 flop); grad / hess: the same count read from the SASS inner loop (58.75 and 46
+# thread-instructions / evaluations).  grad+hess: ncu counters, profiles/r01_cfg3_ncu.md (81.0 FP64
+# instructions, 120.0 flop); grad / hess: the same count read from the SASS inner loop (56.75 and 46
 # instructions).  DESIGN.md sec. 7.  This is what the hardware did -- `roofline.achieved` never claims more.
-FLOPS_PER_EVAL = {"grad+hess": 122.0, "grad": 86.75, "hess": 69.0}
-FP64_INSTR_PER_EVAL = {"grad+hess": 83.0, "grad": 58.75, "hess": 46.0}
+FLOPS_PER_EVAL = {"grad+hess": 120.0, "grad": 84.75, "hess": 69.0}
+FP64_INSTR_PER_EVAL = {"grad+hess": 81.0, "grad": 56.75, "hess": 46.0}
 # SURVEY.md sec. 8(d) canonical count for the cheapest exact formulation it knew (context: this kernel's
 # formulation is cheaper, so evals/s x canonical flops can exceed the FLOP/s peak and is NOT a roofline fraction)
 CANONICAL_FLOPS_PER_EVAL = {"grad+hess": 278.0, "grad": 205.0, "hess": 105.0}
@@ -51,7 +51,7 @@ CANONICAL_FLOPS_PER_EVAL = {"grad+hess": 278.0, "grad": 205.0, "hess": 105.0}
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram bytes (read+write) per launch of the timed kernel from `ncu --set full` (profiles/r01_cfg3_ncu.md:
 # a middle lens chunk of cfg 3 reads and writes the five carried accumulators)
-NCU_TRAFFIC_BYTES = {3: 1.290e9}
+NCU_TRAFFIC_BYTES = {3: 1.289e9}
 
 
 def parse():
