@@ -494,6 +494,32 @@ def test_host_entry_point_matches_device_entry_point():
         assert np.array_equal(host[n], dev[n])
 
 
+def test_host_entry_point_pipelined_pieces_are_bitwise_the_device_result():
+    """Large jobs are cut into row slabs (one map) or model groups (batch) whose device-to-host copies overlap the
+    next piece's computation (lh_api.cu): same bits as the device entry point, ragged slab sizes included."""
+    c = li.config(1)  # 100 dPIE
+    g = li.Grid(x0=c.grid.x0, y0=c.grid.y0, dx=c.grid.dx, nx=1024, ny=1001)  # 16 MB of results -> 3 slabs, ragged
+    dev = run_gpu(c.lenses, g, ("ax", "ay"))
+    host = {n: np.full((g.ny, g.nx), np.nan) for n in ("ax", "ay")}
+    lh.lh_grid_eval_host(c.lenses, 1, c.nlens, g, **host)
+    for n in host:
+        assert np.array_equal(host[n], dev[n])
+    # a model with lens chunks (carry buffer addressed per slab) and the Hessian planes
+    c3 = li.config(3, scale=4)  # 1024 x 1024, 1000 dPIE
+    dev = run_gpu(c3.lenses, c3.grid, ("ay", "kappa", "mu"))
+    host = {n: np.full((c3.grid.ny, c3.grid.nx), np.nan) for n in ("ay", "kappa", "mu")}
+    lh.lh_grid_eval_host(c3.lenses, 1, c3.nlens, c3.grid, **host)
+    for n in host:
+        assert np.array_equal(host[n], dev[n], equal_nan=True)
+    # a batch: 64 models x 300 lenses on 256 x 256 (64 MB of results -> 8 groups of models)
+    c4 = li.config(4, scale=4)
+    dev = run_gpu(c4.lenses, c4.grid, ("ax", "ay"), nmodel=c4.nmodel, nlens=c4.nlens)
+    host = {n: np.full((c4.nmodel, c4.grid.ny, c4.grid.nx), np.nan) for n in ("ax", "ay")}
+    lh.lh_grid_eval_host(c4.lenses, c4.nmodel, c4.nlens, c4.grid, **host)
+    for n in host:
+        assert np.array_equal(host[n], dev[n])
+
+
 def test_fp64_probe_runs():
     flops, secs = lh.lh_fp64_peak_probe(2048)
     assert secs > 0 and 1e12 < flops < 1e14
