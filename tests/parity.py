@@ -80,3 +80,60 @@ def stats_violation(mean_got, var_got, mean_ref, var_ref, nmodel: int):
     vm = float(np.max(np.abs(mean_got - mean_ref)[fin] / am[fin]))
     vv = float(np.max(np.abs(var_got - var_ref)[fin] / np.maximum(av[fin], 5e-324)))
     return vm, vv
+
+
+# ---------------------------------------------------------------- whole-map reports (tests/test_gpu_parity_full.py)
+def plain_ratio_map(got, ref, rel=REL):
+    """|d| / allowed of the plain rule, element by element (same rule as plain_violation)."""
+    got = np.asarray(got, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    allowed = np.maximum(rel * np.abs(ref), rel / REL * FLOOR * np.max(np.abs(ref)))
+    allowed = np.maximum(allowed, 5e-324)
+    with np.errstate(invalid="ignore"):
+        d = np.where(got == ref, 0.0, np.abs(got - ref))
+    return d / allowed
+
+
+def mu_ratio_map(mu_got, mu_ref, kappa_ref, g1_ref, g2_ref, rel=REL):
+    """Element-wise max of the two ratios of the conditioned mu rule (reading R13); non-finite references must
+    be reproduced exactly (ratio 0) or count as a violation (ratio inf)."""
+    mu_got = np.asarray(mu_got, dtype=np.float64)
+    mu_ref = np.asarray(mu_ref, dtype=np.float64)
+    fin = np.isfinite(mu_ref)
+    with np.errstate(invalid="ignore", divide="ignore", over="ignore"):
+        C = ((1.0 - kappa_ref) ** 2 + g1_ref ** 2 + g2_ref ** 2) * np.abs(mu_ref)
+        allowed = np.maximum(rel * np.abs(mu_ref) * np.maximum(1.0, C), 5e-324)
+        r1 = np.where(fin, np.abs(mu_got - mu_ref) / allowed, np.where(mu_got == mu_ref, 0.0, np.inf))
+        r2 = plain_ratio_map(1.0 / mu_got, 1.0 / mu_ref, rel)
+    return np.maximum(r1, r2)
+
+
+def mu_unconditioned_fraction(mu_got, mu_ref, rel=REL):
+    """SURVEY sec. 8(c) pins table, last row: the fraction of pixels that ALSO pass the unconditioned test on mu.
+    Returns (pure relative rule |d| <= rel |mu_ref|, plain rule with the 1e-13 max|mu| floor)."""
+    mu_got = np.asarray(mu_got, dtype=np.float64)
+    mu_ref = np.asarray(mu_ref, dtype=np.float64)
+    with np.errstate(invalid="ignore"):
+        d = np.where(mu_got == mu_ref, 0.0, np.abs(mu_got - mu_ref))
+        pure = float(np.mean(d <= rel * np.abs(mu_ref)))
+        fin = np.isfinite(mu_ref)
+        floor = rel / REL * FLOOR * (np.max(np.abs(mu_ref[fin])) if fin.any() else 0.0)
+        plain = float(np.mean(d <= np.maximum(rel * np.abs(mu_ref), floor)))
+    return pure, plain
+
+
+def report_planes(got: dict, ref: dict, rel=REL):
+    """Whole-map report: name -> {worst, index (flat, of the worst element), n} and for mu the unconditioned
+    pass fractions.  Nothing is asserted here; `worst <= 1` is the pass criterion of check_planes."""
+    rep = {}
+    for n in got:
+        if n == "mu":
+            r = mu_ratio_map(got["mu"], ref["mu"], ref["kappa"], ref["gamma1"], ref["gamma2"], rel)
+        else:
+            r = plain_ratio_map(got[n], ref[n], rel)
+        r = np.where(np.isnan(r), np.inf, r)  # a NaN anywhere is a violation
+        k = int(np.argmax(r))
+        rep[n] = {"worst": float(r.reshape(-1)[k]), "index": k, "n": int(r.size)}
+        if n == "mu":
+            rep[n]["unconditioned_pure"], rep[n]["unconditioned_plain"] = mu_unconditioned_fraction(got["mu"], ref["mu"], rel)
+    return rep

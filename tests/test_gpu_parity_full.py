@@ -1,0 +1,170 @@
+"""Whole-map, FULL-SIZE parity of BASELINE.json configs 1-4: every pixel of every requested plane (-m gpu).
+
+BASELINE.json north_star: "all five configs match the oracle within the stated tolerance"; SURVEY.md sec. 8(d)
+"Oracle timed beside it": the full reference of the large configs is the single-threaded oracle routine run
+over disjoint row ranges on all host cores.  The CUDA side goes through the calls bench.py times
+(lh_grid_eval_batch, lh_grid_gradient_batch) and through the host entry point (lh_grid_eval_host, which must
+be bit-identical to the device planes).  cfg 0 is compared whole in test_gpu_parity.py.
+
+Per plane the test asserts worst |d|/allowed <= 1 (tests/parity.py; mu by the conditioned rule, reading R13,
+PAPER.md:66) and reports -- SURVEY.md sec. 8(c) pins table, last row -- the fraction of pixels that ALSO pass
+the unconditioned 1e-11 test on mu.  The numbers are appended to $LH_PARITY_REPORT (default
+gpurun_out/parity_full.jsonl when that directory exists); profiles/r02_parity_full.md is made from that file.
+
+Time: at the oracle's measured 8.6e6 evals/s per core the references cost about 1 s / 15 s / 2 min / 2.5 min on
+16 cores.  If the host is so slow that a reference would take more than LH_PARITY_BUDGET_S seconds (default
+420), rows are strided (every k-th row of every model, all columns) and the report says so -- the assertion then
+covers the evaluated rows only.
+"""
+import json
+import os
+import time
+
+import numpy as np
+import pytest
+
+import lens_inputs as li
+import oracle
+import paper_2004_06352_b200 as lh
+from parity import report_planes
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+NTHREADS = max(1, os.cpu_count() or 1)
+BUDGET_S = float(os.environ.get("LH_PARITY_BUDGET_S", "420"))
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _report_path():
+    p = os.environ.get("LH_PARITY_REPORT")
+    if p:
+        return p
+    d = os.path.join(ROOT, "gpurun_out")
+    return os.path.join(d, "parity_full.jsonl") if os.path.isdir(d) else None
+
+
+def _emit(rec):
+    line = json.dumps(rec)
+    print("PARITY_FULL " + line)
+    p = _report_path()
+    if p:
+        with open(p, "a") as f:
+            f.write(line + "\n")
+
+
+def _need(names):
+    need = set(names)
+    if "mu" in need:
+        need |= {"kappa", "gamma1", "gamma2"}
+    return tuple(sorted(need))
+
+
+def _row_stride(evals):
+    """1 when the full reference fits the time budget on this host, else the row stride that does."""
+    g = li.Grid(x0=-1.0, y0=-1.0, dx=0.01, nx=256, ny=NTHREADS * 4)
+    L = li.config(1).lenses
+    t0 = time.perf_counter()
+    oracle.grid(L, g.x0, g.y0, g.dx, g.nx, g.ny, planes=("ax", "kappa"), threads=NTHREADS)
+    rate = g.npix * len(L) / (time.perf_counter() - t0)
+    est = evals / rate
+    return max(1, int(np.ceil(est / BUDGET_S))), rate
+
+
+def _reference(lenses, g, names, stride):
+    """Oracle planes on rows 0, stride, 2 stride, ... (all rows when stride == 1), each [nrows, nx]."""
+    need = _need(names)
+    if stride == 1:
+        return oracle.grid(lenses, g.x0, g.y0, g.dx, g.nx, g.ny, planes=need, threads=NTHREADS), slice(None)
+    rows = np.arange(0, g.ny, stride)
+    # the strided rows as lists of points: same per-pixel routine, same coordinates x0 + i dx, y0 + j dx;
+    # chunks of rows fan out over host threads (ctypes drops the GIL)
+    from concurrent.futures import ThreadPoolExecutor
+
+    xs = g.x0 + np.arange(g.nx) * g.dx
+
+    def run(chunk):
+        X = np.ascontiguousarray(np.broadcast_to(xs, (len(chunk), g.nx)))
+        Y = np.ascontiguousarray(np.broadcast_to((g.y0 + chunk * g.dx)[:, None], (len(chunk), g.nx)))
+        return oracle.points(lenses, X, Y, planes=need)
+
+    chunks = [c for c in np.array_split(rows, min(len(rows), NTHREADS * 4)) if len(c)]
+    with ThreadPoolExecutor(NTHREADS) as ex:
+        parts = list(ex.map(run, chunks))
+    return {n: np.concatenate([p[n] for p in parts]) for n in need}, rows
+
+
+def _check_and_report(cfg_idx, c, got_model, lenses, what, stride, rate, model=None):
+    g = c.grid
+    t0 = time.perf_counter()
+    ref, rows = _reference(lenses, g, c.outputs, stride)
+    t_ref = time.perf_counter() - t0
+    got = {n: got_model[n][rows] for n in c.outputs}
+    rep = report_planes(got, ref)
+    rec = {"cfg": cfg_idx, "what": what, "model": model, "grid": [g.nx, g.ny], "nlens": len(lenses),
+           "row_stride": stride, "pixels_compared": int(next(iter(got.values())).size), "oracle_s": round(t_ref, 2),
+           "oracle_threads": NTHREADS, "planes": {}}
+    for n, r in rep.items():
+        k = r["index"]
+        jj = k // g.nx
+        j = jj if stride == 1 else int(np.arange(0, g.ny, stride)[jj])
+        rec["planes"][n] = {"worst_ratio": r["worst"], "pixel_ij": [int(k % g.nx), int(j)]}
+        if n == "mu":
+            rec["planes"][n]["frac_pass_unconditioned_1e-11_pure_relative"] = r["unconditioned_pure"]
+            rec["planes"][n]["frac_pass_unconditioned_plain_rule"] = r["unconditioned_plain"]
+            det_small = float(np.mean(np.abs(1.0 / ref["mu"]) < 1e-3))
+            rec["planes"][n]["frac_pixels_absdet_below_1e-3"] = det_small
+    bad = {n: r["worst"] for n, r in rep.items() if not r["worst"] <= 1.0}
+    return rec, bad
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3])
+def test_full_size_whole_map(idx):
+    """cfg 1, 2, 3: every pixel of every requested plane, through lh_grid_eval_batch (the call bench.py times)
+    and through lh_grid_eval_host (bit-identical planes in host memory)."""
+    c = li.config(idx)
+    g = c.grid
+    stride, rate = _row_stride(c.evals)
+    out = {n: torch.full((1, g.ny, g.nx), float("nan"), dtype=torch.float64, device="cuda") for n in c.outputs}
+    lh.lh_grid_eval_batch(c.lenses, 1, c.nlens, g, **out)
+    torch.cuda.synchronize()
+    got = {n: v[0].cpu().numpy() for n, v in out.items()}
+    del out
+    rec, bad = _check_and_report(idx, c, got, c.lenses, "lh_grid_eval_batch", stride, rate)
+    # host entry point: pageable numpy planes, pipelined row slabs -- must be the same bits
+    host = {n: np.full((g.ny, g.nx), np.nan) for n in c.outputs}
+    lh.lh_grid_eval_host(c.lenses, 1, c.nlens, g, **host)
+    rec["lh_grid_eval_host_bitwise_equal"] = bool(all(np.array_equal(host[n], got[n], equal_nan=True) for n in host))
+    _emit(rec)
+    assert not bad, f"{c.name}: whole-map parity violated (|d|/allowed): {bad}"
+    assert rec["lh_grid_eval_host_bitwise_equal"]
+    for n in got:
+        assert not np.isnan(got[n]).any()
+
+
+def test_full_size_whole_batch_cfg4():
+    """cfg 4: every pixel of both planes of all 64 models, through lh_grid_gradient_batch (one call)."""
+    c = li.config(4)
+    g = c.grid
+    stride, rate = _row_stride(c.evals)
+    out = {n: torch.full((c.nmodel, g.ny, g.nx), float("nan"), dtype=torch.float64, device="cuda") for n in c.outputs}
+    lh.lh_grid_gradient_batch(c.lenses, c.nmodel, c.nlens, g, out["ax"], out["ay"])
+    torch.cuda.synchronize()
+    assert not torch.isnan(out["ax"]).any() and not torch.isnan(out["ay"]).any()
+    worst = {n: (0.0, None, None) for n in c.outputs}
+    t_ref, npx, bad_all = 0.0, 0, {}
+    for m in range(c.nmodel):
+        got = {n: out[n][m].cpu().numpy() for n in c.outputs}
+        rec, bad = _check_and_report(4, c, got, c.lenses[m * c.nlens:(m + 1) * c.nlens], "lh_grid_gradient_batch",
+                                     stride, rate, model=m)
+        t_ref += rec["oracle_s"]
+        npx += rec["pixels_compared"]
+        for n, p in rec["planes"].items():
+            if p["worst_ratio"] > worst[n][0]:
+                worst[n] = (p["worst_ratio"], m, p["pixel_ij"])
+        if bad:
+            bad_all[m] = bad
+    _emit({"cfg": 4, "what": "lh_grid_gradient_batch", "grid": [g.nx, g.ny], "nlens": c.nlens, "nmodel": c.nmodel,
+           "row_stride": stride, "pixels_compared": npx, "oracle_s": round(t_ref, 2), "oracle_threads": NTHREADS,
+           "planes": {n: {"worst_ratio": w[0], "model": w[1], "pixel_ij": w[2]} for n, w in worst.items()}})
+    assert not bad_all, f"{c.name}: whole-batch parity violated: {bad_all}"
