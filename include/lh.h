@@ -35,13 +35,16 @@
  *              calling host thread (default: the legacy default stream) and the
  *              call returns without synchronising the device.  (The *_host entry
  *              points synchronise that stream before they return.)
- *   errors     0 on success.  A negative code on failure, in which case no
- *              output element has been written; lh_last_error() gives a message.
+ *   errors     0 on success, a negative code on failure; lh_last_error() gives a message.
+ *              LH_EINVAL (a bad argument: every argument, every lens of every model and every
+ *              constraint is checked first): nothing was enqueued, no output element written.
+ *              LH_ECUDA (a CUDA call failed): work may already be enqueued; outputs undefined.
  *              No exception or abort crosses this boundary.
  *   nlens = 0  is valid: alpha = 0, a_ij = 0, kappa = gamma = 0, mu = 1.
- *   range      lengths (positions, radii, pixel size) may use any unit, but all of them must lie within about
- *              1e+-35 of one another: the kernel takes ONE reciprocal of a product of four squared lengths
- *              per evaluation and that product must stay inside the double range.
+ *   range      lengths (positions, radii, pixel size) may use any unit in which all of them lie between about
+ *              1e-20 and 1e+17: the kernel takes ONE reciprocal of a product of two squared and two cubed lengths
+ *              of the scaled lens frame (scale factor <= 2^40) per evaluation, and that
+ *              product must stay inside the double range.
  *   IEEE       mu = +-inf where det A^-1 == 0 exactly.  A pixel that coincides
  *              exactly with the centre of an SIS gets zero contribution from it.
  */
@@ -71,7 +74,7 @@ typedef struct {
     double theta;       /* position angle of the major axis, CCW from +x; ignored for SIS */
     double rcore;       /* dPIE: 0 < rcore < rcut; NSIE: > 0; SIS: ignored */
     double rcut;        /* dPIE only */
-    double b0;          /* = (D_ls/D_s) 6 pi (sigma/c)^2 in arcsec, finite (SIS: |alpha| = b0) */
+    double b0;          /* = (D_ls/D_s) 6 pi (sigma/c)^2 in arcsec, finite and >= 0 (SIS: |alpha| = b0) */
 } lh_lens;
 
 /* Regular grid with square pixels: pixel (i, j) at (x0 + i*dx, y0 + j*dx). */
@@ -89,7 +92,7 @@ typedef struct {
 
 /* alpha_x, alpha_y on the grid (eq. 10).  Both planes required.
  * LH_EINVAL: NULL pointer, nlens < 0, nx or ny <= 0, nx*ny >= 2^40, dx <= 0 or
- * non-finite x0/y0/dx, unknown lens type, non-finite parameter, e-hat outside [0,1),
+ * non-finite x0/y0/dx, unknown lens type, non-finite parameter, b0 < 0, e-hat outside [0,1),
  * dPIE with rcore <= 0 or rcut <= rcore, NSIE with rcore <= 0, output pointer that
  * is not device memory or not 8-byte aligned. */
 int lh_grid_gradient(const lh_lens *lenses, int nlens, const lh_grid *g, double *out_ax, double *out_ay);
@@ -247,20 +250,6 @@ int lh_fp64_peak_probe(int iters, double *flops_per_s, double *seconds);
  *      5  1/a via the shared-seed pair (a, b)     6  1/a via the shared-seed quadruple (a, b, a+b, 2b)
  * No CUDA call is made.  LH_EINVAL for an unknown fn or a NULL pointer (b may be NULL for fn 0-2). */
 int lh_math_host_eval(int fn, const double *a, const double *b, size_t n, double *out);
-
-/* Diagnostic behind DESIGN.md sec. 7 (the dispatch-cost model the kernel is written against).
- * One group = 12 independent warp-wide FP64 instructions (+ `extra` other instructions); every
- * warp runs `iters` groups with `warps_per_subpartition` (1..16) warps resident per SM
- * sub-partition on every SM.  *cycles_per_group = elapsed time x max SM clock / (iters x
- * warps_per_subpartition): 24 means one FP64 instruction per 2 cycles.
- *   variant 0  FMA with immediate operands      1  FMA, three distinct vector registers
- *           2  FMA, two distinct registers      3  MUL, two registers
- *           4  FMA, one uniform operand loaded from the kernel parameters
- *           5  FMA, one register shared by consecutive instructions
- *   variant 10/11/12/13  a MUL stream plus `extra` (0, 2, 4, 8) LOP3 / FFMA /
- *           MUFU.RCP64H+MOV / LDS instructions per group.
- * Synchronises the set stream.  LH_EINVAL for an unknown variant/extra. */
-int lh_fp64_issue_probe(int variant, int extra, int warps_per_subpartition, int iters, double *cycles_per_group);
 
 /* "lh <major>.<minor> sm_100a" */
 const char *lh_version(void);

@@ -256,7 +256,17 @@ void orc_source_plane(const double *ax, const double *ay, double x0, double y0, 
         }
 }
 
+static double min3(double a, double b, double c) { return fmin(fmin(a, b), c); }
+static double max3(double a, double b, double c) { return fmax(fmax(a, b), c); }
+
+/* Reading R22: S is inside the closed triangle ABC iff it lies in the closed bounding box of
+ * the three vertices AND d != 0, u >= 0, v >= 0, u + v <= 1.  The box is part of the definition: a point of a
+ * closed triangle is always inside the box of its vertices, but the ROUNDED barycentric test alone can accept a
+ * point one ulp outside an extreme vertex (S - A rounds to B - A, u = 1, v = 0); the box makes that case a miss. */
 static int tri_test(const double A[2], const double B[2], const double C[2], const double S[2], double *u, double *v) {
+    if (S[0] < min3(A[0], B[0], C[0]) || S[0] > max3(A[0], B[0], C[0]) || S[1] < min3(A[1], B[1], C[1]) ||
+        S[1] > max3(A[1], B[1], C[1]))
+        return 0;
     const double e1x = B[0] - A[0], e1y = B[1] - A[1];
     const double e2x = C[0] - A[0], e2y = C[1] - A[1];
     const double sx = S[0] - A[0], sy = S[1] - A[1];

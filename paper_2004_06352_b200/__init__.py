@@ -8,7 +8,7 @@ missing -- there is no CPU fallback (and it never imports `oracle`).
 Names mirror the C ABI one to one:
     lh_grid_gradient, lh_grid_hessian, lh_lens_maps, lh_grid_gradient_batch,
     lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_grid_stats_batch, lh_pack_model, lh_set_stream,
-    lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_fp64_issue_probe, lh_math_host_eval, lh_version
+    lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_math_host_eval, lh_version
 Outputs may be torch CUDA tensors (float64, contiguous), anything with a
 `data_ptr()`, or raw integer device addresses.
 """
@@ -16,6 +16,7 @@ from __future__ import annotations
 
 import ctypes as C
 import os
+import sys
 
 import numpy as np
 
@@ -89,8 +90,6 @@ def _load():
         L.lh_fp64_peak_probe.argtypes = [ci, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.lh_math_host_eval.argtypes = [ci, vp, vp, C.c_size_t, vp]
         L.lh_math_host_eval.restype = ci
-        L.lh_fp64_issue_probe.argtypes = [ci, ci, ci, ci, C.POINTER(C.c_double)]
-        L.lh_fp64_issue_probe.restype = ci
         L.lh_version.restype = C.c_char_p
         for f in ("lh_grid_gradient", "lh_grid_hessian", "lh_lens_maps", "lh_grid_gradient_batch", "lh_grid_eval",
                   "lh_grid_eval_batch", "lh_grid_eval_host", "lh_set_stream", "lh_fp64_peak_probe"):
@@ -114,7 +113,10 @@ def _grid(g) -> lh_grid:
     return lh_grid(float(g.x0), float(g.y0), float(g.dx), int(g.nx), int(g.ny))
 
 
-def _dev_ptr(t):
+def _dev_ptr(t, count=None):
+    """Device address of an output / input buffer.  `count`: the number of float64 elements the call will write
+    (or read) there; a tensor that is smaller, or lives on another device than the current one, is refused HERE --
+    the C ABI only sees an address and cannot tell (it would be an out-of-bounds write on the device)."""
     if t is None:
         return None
     if isinstance(t, int):
@@ -124,6 +126,12 @@ def _dev_ptr(t):
             raise TypeError("output tensors must be contiguous")
         if hasattr(t, "dtype") and "float64" not in str(t.dtype):
             raise TypeError("output tensors must be float64")
+        if count is not None and hasattr(t, "numel") and int(t.numel()) < count:
+            raise ValueError(f"tensor of {int(t.numel())} elements where the call needs {count}")
+        if getattr(t, "is_cuda", False):
+            torch = sys.modules.get("torch")
+            if torch is not None and t.device.index is not None and t.device.index != torch.cuda.current_device():
+                raise ValueError(f"tensor on cuda:{t.device.index} but the current device is cuda:{torch.cuda.current_device()}")
         return t.data_ptr()
     raise TypeError(f"cannot take a device pointer from {type(t)}")
 
@@ -133,41 +141,49 @@ def _check(rc: int):
         raise LhError(rc, _load().lh_last_error().decode())
 
 
-def _outputs(planes: dict, to_ptr) -> lh_outputs:
+def _outputs(planes: dict, to_ptr, count=None) -> lh_outputs:
     bad = set(planes) - set(PLANES)
     if bad:
         raise KeyError(f"unknown planes {sorted(bad)}")
-    return lh_outputs(**{n: to_ptr(planes.get(n)) for n in PLANES})
+    return lh_outputs(**{n: to_ptr(planes.get(n), count) for n in PLANES})
+
+
+def _npix(grid, nmodel=1) -> int:
+    return int(grid.nx) * int(grid.ny) * int(nmodel)
 
 
 # ---------------------------------------------------------------- the C ABI, name for name
 def lh_grid_gradient(lenses, grid, out_ax, out_ay):
     a, p, n = _lenses_ptr(lenses)
-    _check(_load().lh_grid_gradient(p, n, C.byref(_grid(grid)), _dev_ptr(out_ax), _dev_ptr(out_ay)))
+    k = _npix(grid)
+    _check(_load().lh_grid_gradient(p, n, C.byref(_grid(grid)), _dev_ptr(out_ax, k), _dev_ptr(out_ay, k)))
 
 
 def lh_grid_hessian(lenses, grid, a11, a12, a22):
     a, p, n = _lenses_ptr(lenses)
-    _check(_load().lh_grid_hessian(p, n, C.byref(_grid(grid)), _dev_ptr(a11), _dev_ptr(a12), _dev_ptr(a22)))
+    k = _npix(grid)
+    _check(_load().lh_grid_hessian(p, n, C.byref(_grid(grid)), _dev_ptr(a11, k), _dev_ptr(a12, k), _dev_ptr(a22, k)))
 
 
 def lh_lens_maps(lenses, grid, kappa, gamma1, gamma2, mu):
     a, p, n = _lenses_ptr(lenses)
-    _check(_load().lh_lens_maps(p, n, C.byref(_grid(grid)), _dev_ptr(kappa), _dev_ptr(gamma1), _dev_ptr(gamma2),
-                                _dev_ptr(mu)))
+    k = _npix(grid)
+    _check(_load().lh_lens_maps(p, n, C.byref(_grid(grid)), _dev_ptr(kappa, k), _dev_ptr(gamma1, k), _dev_ptr(gamma2, k),
+                                _dev_ptr(mu, k)))
 
 
 def lh_grid_gradient_batch(lenses, nmodel, nlens, grid, out_ax, out_ay):
     a, p, n = _lenses_ptr(lenses)
     if n != nmodel * nlens:
         raise ValueError("len(lenses) != nmodel*nlens")
-    _check(_load().lh_grid_gradient_batch(p, nmodel, nlens, C.byref(_grid(grid)), _dev_ptr(out_ax), _dev_ptr(out_ay)))
+    k = _npix(grid, nmodel)
+    _check(_load().lh_grid_gradient_batch(p, nmodel, nlens, C.byref(_grid(grid)), _dev_ptr(out_ax, k), _dev_ptr(out_ay, k)))
 
 
 def lh_grid_eval(lenses, grid, **planes):
     """planes: any of ax, ay, a11, a12, a22, kappa, gamma1, gamma2, mu = device tensor."""
     a, p, n = _lenses_ptr(lenses)
-    o = _outputs(planes, _dev_ptr)
+    o = _outputs(planes, _dev_ptr, _npix(grid))
     _check(_load().lh_grid_eval(p, n, C.byref(_grid(grid)), C.byref(o)))
 
 
@@ -178,8 +194,9 @@ def lh_chi2(lenses, grid, constraints, nsources: int, chi2, predicted=None, sour
     c = np.ascontiguousarray(constraints)
     if c.dtype.itemsize != 32:
         raise TypeError("constraints must be an array of 32-byte lh_constraint records")
-    _check(_load().lh_chi2(p, n, C.byref(_grid(grid)), c.ctypes.data, c.size, int(nsources), _dev_ptr(chi2),
-                           _dev_ptr(predicted), _dev_ptr(sources), None if nimages is None else nimages.data_ptr()))
+    _check(_load().lh_chi2(p, n, C.byref(_grid(grid)), c.ctypes.data, c.size, int(nsources), _dev_ptr(chi2, 1),
+                           _dev_ptr(predicted, 2 * c.size), _dev_ptr(sources, 2 * int(nsources)),
+                           None if nimages is None else nimages.data_ptr()))
 
 
 def lh_points_eval(lenses, xs, ys, **planes):
@@ -188,14 +205,14 @@ def lh_points_eval(lenses, xs, ys, **planes):
     npts = int(xs.numel()) if hasattr(xs, "numel") else None
     if npts is None or npts != int(ys.numel()):
         raise ValueError("xs and ys must be device tensors of equal length")
-    o = _outputs(planes, _dev_ptr)
-    _check(_load().lh_points_eval(p, n, _dev_ptr(xs), _dev_ptr(ys), npts, C.byref(o)))
+    o = _outputs(planes, _dev_ptr, npts)
+    _check(_load().lh_points_eval(p, n, _dev_ptr(xs, npts), _dev_ptr(ys, npts), npts, C.byref(o)))
 
 
 def lh_grid_eval_rows(lenses, grid, j0: int, nrows: int, **planes):
     """Rows [j0, j0+nrows) of the grid into planes of shape [nrows, nx] (the multi-GPU row-slab primitive)."""
     a, p, n = _lenses_ptr(lenses)
-    o = _outputs(planes, _dev_ptr)
+    o = _outputs(planes, _dev_ptr, int(nrows) * int(grid.nx))
     _check(_load().lh_grid_eval_rows(p, n, C.byref(_grid(grid)), int(j0), int(nrows), C.byref(o)))
 
 
@@ -203,7 +220,7 @@ def lh_grid_eval_batch(lenses, nmodel, nlens, grid, **planes):
     a, p, n = _lenses_ptr(lenses)
     if n != nmodel * nlens:
         raise ValueError("len(lenses) != nmodel*nlens")
-    o = _outputs(planes, _dev_ptr)
+    o = _outputs(planes, _dev_ptr, _npix(grid, nmodel))
     _check(_load().lh_grid_eval_batch(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(o)))
 
 
@@ -213,7 +230,7 @@ def lh_grid_eval_batch_shared(shared, varying, nmodel, nvar, grid, **planes):
     va, vpn, vn = _lenses_ptr(varying)
     if vn != nmodel * nvar:
         raise ValueError("len(varying) != nmodel*nvar")
-    o = _outputs(planes, _dev_ptr)
+    o = _outputs(planes, _dev_ptr, _npix(grid, nmodel))
     _check(_load().lh_grid_eval_batch_shared(sp, sn, vpn, nmodel, nvar, C.byref(_grid(grid)), C.byref(o)))
 
 
@@ -222,8 +239,8 @@ def lh_grid_stats_batch(lenses, nmodel, nlens, grid, mean: dict, var: dict | Non
     a, p, n = _lenses_ptr(lenses)
     if n != nmodel * nlens:
         raise ValueError("len(lenses) != nmodel*nlens")
-    om = _outputs(mean, _dev_ptr)
-    ov = _outputs(var, _dev_ptr) if var else None
+    om = _outputs(mean, _dev_ptr, _npix(grid))
+    ov = _outputs(var, _dev_ptr, _npix(grid)) if var else None
     _check(_load().lh_grid_stats_batch(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(om),
                                        C.byref(ov) if ov is not None else None))
 
@@ -233,7 +250,8 @@ LH_IMAGE_DTYPE = np.dtype([("source", "<i4"), ("_pad", "<i4"), ("triangle", "<i8
 
 def lh_source_plane(ax, ay, grid, bx=None, by=None):
     """beta = theta - alpha on the grid; device planes [ny, nx]."""
-    _check(_load().lh_source_plane(_dev_ptr(ax), _dev_ptr(ay), C.byref(_grid(grid)), _dev_ptr(bx), _dev_ptr(by)))
+    k = _npix(grid)
+    _check(_load().lh_source_plane(_dev_ptr(ax, k), _dev_ptr(ay, k), C.byref(_grid(grid)), _dev_ptr(bx, k), _dev_ptr(by, k)))
 
 
 def lh_delens_grid(ax, ay, grid, sources, images, max_images: int, count):
@@ -241,11 +259,15 @@ def lh_delens_grid(ax, ay, grid, sources, images, max_images: int, count):
     torch uint8 tensor of 32*max_images bytes, view it with LH_IMAGE_DTYPE on the host); count: device int64[1]."""
     src = np.ascontiguousarray(sources, dtype=np.float64).reshape(-1, 2)
 
-    def raw(t):  # any device buffer: only the address is taken
-        return None if t is None else (t if isinstance(t, int) else t.data_ptr())
+    def raw(t, nbytes):  # any device buffer: only the address is taken, the size in bytes is checked
+        if t is None or isinstance(t, int):
+            return t
+        if hasattr(t, "numel") and hasattr(t, "element_size") and int(t.numel()) * int(t.element_size()) < nbytes:
+            raise ValueError(f"buffer of {int(t.numel()) * int(t.element_size())} bytes where the call needs {nbytes}")
+        return t.data_ptr()
 
-    _check(_load().lh_delens_grid(_dev_ptr(ax), _dev_ptr(ay), C.byref(_grid(grid)), src.ctypes.data, len(src),
-                                  raw(images), int(max_images), raw(count)))
+    _check(_load().lh_delens_grid(_dev_ptr(ax, _npix(grid)), _dev_ptr(ay, _npix(grid)), C.byref(_grid(grid)), src.ctypes.data, len(src),
+                                  raw(images, 32 * int(max_images)), int(max_images), raw(count, 8)))
 
 
 def lh_grid_eval_host(lenses, nmodel, nlens, grid, **host_planes):
@@ -255,18 +277,26 @@ def lh_grid_eval_host(lenses, nmodel, nlens, grid, **host_planes):
     if n != nmodel * nlens:
         raise ValueError("len(lenses) != nmodel*nlens")
 
-    def host_ptr(v):
+    def host_ptr(v, count):
         if v is None:
             return None
         if isinstance(v, np.ndarray):
             if v.dtype != np.float64 or not v.flags.c_contiguous:
                 raise TypeError("host planes must be C-contiguous float64")
+            if v.size < count:
+                raise ValueError(f"host plane of {v.size} elements where the call needs {count}")
             return v.ctypes.data
         if hasattr(v, "data_ptr"):  # e.g. a pinned torch CPU tensor
+            if getattr(v, "is_cuda", False):
+                raise TypeError("lh_grid_eval_host takes HOST planes")
+            if "float64" not in str(v.dtype) or not v.is_contiguous():
+                raise TypeError("host planes must be contiguous float64")
+            if int(v.numel()) < count:
+                raise ValueError(f"host plane of {int(v.numel())} elements where the call needs {count}")
             return v.data_ptr()
         raise TypeError(f"cannot take a host pointer from {type(v)}")
 
-    o = _outputs(host_planes, host_ptr)
+    o = _outputs(host_planes, host_ptr, _npix(grid, nmodel))
     _check(_load().lh_grid_eval_host(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(o)))
 
 
@@ -315,13 +345,6 @@ def lh_math_host_eval(fn: int, a, b=None):
     _check(_load().lh_math_host_eval(int(fn), a.ctypes.data, None if bb is None else bb.ctypes.data, a.size,
                                      out.ctypes.data))
     return out
-
-
-def lh_fp64_issue_probe(variant: int, extra: int = 0, warps_per_subpartition: int = 8, iters: int = 20000) -> float:
-    """Dispatch cycles per group of 12 FP64 instructions (+ `extra` others); see include/lh.h."""
-    c = C.c_double()
-    _check(_load().lh_fp64_issue_probe(int(variant), int(extra), int(warps_per_subpartition), int(iters), C.byref(c)))
-    return c.value
 
 
 def lh_version() -> str:

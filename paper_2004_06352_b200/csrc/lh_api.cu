@@ -56,6 +56,11 @@ struct DeviceState {
     double *d_sink = nullptr;
     char *d_chi = nullptr;  // scratch of lh_chi2 (deflection planes, constraint arrays, sources, images)
     size_t chi_bytes = 0;
+    cudaEvent_t ev_chi = nullptr;  // end of the last lh_chi2 that used d_chi, on chi_stream (same protocol as d_carry)
+    cudaStream_t chi_stream = nullptr;
+    bool chi_busy = false;
+    cudaStream_t aux_stream = nullptr;  // second launch chain of batches of chunked models (lh_kernels.cu)
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
 struct Context {
@@ -156,16 +161,13 @@ struct EvalOpts {
     int nshared = 0;
     int j0 = 0, nrows = -1;           // rows [j0, j0 + nrows) of the grid only (dev_out point at row j0); default all
     const double *px = nullptr, *py = nullptr;  // DEVICE: evaluate at these g->nx points instead of a grid (g->ny = 1)
+    // >= 0: the models were validated and packed into ctx.h_table / ctx.h_ranges by pack_all() already and this job
+    // evaluates `nmodel` of them starting at model `packed0` (`lenses` is then not read)
+    int packed0 = -1;
 };
 
-int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *dev_out[NPLANES],
-                const EvalOpts &opt = EvalOpts()) {
-    double **dev_m2 = opt.m2;
-    const lh_lens *shared = opt.shared;
-    const int nshared = opt.nshared, j0 = opt.j0;
-    int nrows = opt.nrows;
-    if (nrows < 0) nrows = g->ny;
-    // a1: pack on the host (validates; nothing is enqueued if any lens is rejected)
+// a1 for a whole call: validate + pack nmodel x nlens lenses into ctx.h_table / ctx.h_ranges.  Nothing is enqueued.
+int pack_all(const lh_lens *lenses, int nmodel, int nlens) {
     try {
         ctx.h_table.resize((size_t)nmodel * (size_t)nlens);
         ctx.h_ranges.resize((size_t)nmodel);
@@ -176,6 +178,37 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
         if (lh::pack_model(lenses + (size_t)m * nlens, nlens, ctx.h_table.data() + (size_t)m * nlens,
                            ctx.h_ranges.data() + m, ctx.err, sizeof(ctx.err), m) != 0)
             return LH_EINVAL;  // message already written
+    }
+    return LH_OK;
+}
+
+// The carry buffer of this device: at least `need` bytes, safe to use on stream `s` once this returns.
+int ensure_carry(size_t need, cudaStream_t s) {
+    if (!DS().ev_done) CU(cudaEventCreateWithFlags(&DS().ev_done, cudaEventDisableTiming));
+    if (need > DS().carry_bytes) {
+        if (DS().busy) CU(cudaEventSynchronize(DS().ev_done));  // the old buffer is no longer in use
+        if (DS().d_carry) cudaFree(DS().d_carry);
+        DS().d_carry = nullptr;
+        DS().carry_bytes = 0;
+        CU(cudaMalloc(&DS().d_carry, need));
+        DS().carry_bytes = need;
+    }
+    if (need && DS().busy && DS().last_stream != s) CU(cudaStreamWaitEvent(s, DS().ev_done, 0));
+    return LH_OK;
+}
+
+int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *dev_out[NPLANES],
+                const EvalOpts &opt = EvalOpts()) {
+    double **dev_m2 = opt.m2;
+    const lh_lens *shared = opt.shared;
+    const int nshared = opt.nshared, j0 = opt.j0;
+    int nrows = opt.nrows;
+    if (nrows < 0) nrows = g->ny;
+    // a1: pack on the host (validates; nothing is enqueued if any lens is rejected)
+    const int m_first = opt.packed0 >= 0 ? opt.packed0 : 0;
+    if (opt.packed0 < 0) {
+        int rc = pack_all(lenses, nmodel, nlens);
+        if (rc) return rc;
     }
 
     lh::ModelRanges shared_ranges = {};
@@ -190,18 +223,20 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     }
 
     cudaStream_t s = ctx.stream;
-    if (!DS().ev_done) CU(cudaEventCreateWithFlags(&DS().ev_done, cudaEventDisableTiming));
-    const size_t carry_need =
+    const size_t carry_one =
         (nlens > lh::LAUNCH_RECORDS || nshared > 0) ? (size_t)5 * g->nx * g->ny * sizeof(double) : 0;
-    if (carry_need > DS().carry_bytes) {
-        if (DS().busy) CU(cudaEventSynchronize(DS().ev_done));  // the old buffer is no longer in use
-        if (DS().d_carry) cudaFree(DS().d_carry);
-        DS().d_carry = nullptr;
-        DS().carry_bytes = 0;
-        CU(cudaMalloc(&DS().d_carry, carry_need));
-        DS().carry_bytes = carry_need;
+    // batches of chunked models run as two interleaved launch chains, each with a carry buffer of its own
+    const bool two_chains = nlens > lh::LAUNCH_RECORDS && nmodel > 1 && !dev_m2 && nshared == 0;
+    const size_t carry_need = carry_one * (two_chains ? 2 : 1);
+    if (two_chains && !DS().aux_stream) {
+        CU(cudaStreamCreateWithFlags(&DS().aux_stream, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&DS().ev_fork, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&DS().ev_join, cudaEventDisableTiming));
     }
-    if (carry_need && DS().busy && DS().last_stream != s) CU(cudaStreamWaitEvent(s, DS().ev_done, 0));
+    {
+        int rc = ensure_carry(carry_need, s);
+        if (rc) return rc;
+    }
 
     int dev = 0;
     CU(cudaGetDevice(&dev));
@@ -209,8 +244,8 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     lh::EvalJob J;
     J.math = device_math_tables(dev, &terr);
     if (!J.math) return fail(LH_ECUDA, "math tables: %s", cudaGetErrorString(terr));
-    J.table = ctx.h_table.data();
-    J.ranges = ctx.h_ranges.data();
+    J.table = ctx.h_table.data() + (size_t)m_first * nlens;
+    J.ranges = ctx.h_ranges.data() + m_first;
     J.nlens = nlens;
     J.nmodel = nmodel;
     J.shared_table = nshared > 0 ? ctx.h_shared.data() : nullptr;
@@ -229,6 +264,12 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     // carry is laid out like the planes it serves: a slab of FULL-size planes (nrows < g->ny) uses the slab's rows
     // of a full-size carry; a stand-alone slab (lh_grid_eval_rows: g->ny == nrows) uses a carry of its own size
     J.carry = DS().d_carry ? DS().d_carry + (nrows != g->ny ? (size_t)j0 * g->nx : 0) : nullptr;
+    if (two_chains) {
+        J.carry2 = DS().d_carry + carry_one / sizeof(double);
+        J.aux = DS().aux_stream;
+        J.ev_fork = DS().ev_fork;
+        J.ev_join = DS().ev_join;
+    }
     CU(lh::launch_eval(J, s, &ctx.launches));
     if (carry_need) {
         CU(cudaEventRecord(DS().ev_done, s));
@@ -465,15 +506,8 @@ int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constra
     if (predicted && (rc = check_device_ptr(predicted, "predicted"))) return rc;
     if (sources && (rc = check_device_ptr(sources, "sources"))) return rc;
     if (nimages && (rc = check_device_ptr(reinterpret_cast<double *>(nimages), "nimages"))) return rc;
-    {  // validate the lens list before anything is enqueued
-        lh::ModelRanges r;
-        try {
-            ctx.h_table.resize((size_t)nlens);
-        } catch (const std::bad_alloc &) {
-            return fail(LH_EINVAL, "out of host memory packing %d lenses", nlens);
-        }
-        if (lh::pack_model(lenses, nlens, ctx.h_table.data(), &r, ctx.err, sizeof(ctx.err), 0) != 0) return LH_EINVAL;
-    }
+    // validate and pack the lens list once; both evaluations below reuse the packed table
+    if ((rc = pack_all(lenses, 1, nlens))) return rc;
 
     // scratch layout (all 16-byte aligned)
     const size_t npix = (size_t)g->nx * g->ny;
@@ -484,15 +518,34 @@ int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constra
                  o_bay = o_bax + al((size_t)K * 8 + 16), o_term = o_bay + al((size_t)K * 8 + 16),
                  o_src = o_term + al((size_t)K * 8 + 16), o_cnt = o_src + al((size_t)N * 16 + 16), o_im = o_cnt + 16,
                  total = o_im + (size_t)cap * sizeof(lh_image);
+    cudaStream_t s = ctx.stream;
+    // Everything that can fail for lack of memory is obtained BEFORE the first enqueue: the scratch buffer, the carry
+    // buffer of the larger of the two evaluations and the math tables.  The scratch is cached per device and reused
+    // across calls: stream order protects it on one stream, ev_chi + cudaStreamWaitEvent across a stream change, and
+    // it is only freed after the last call that used it has finished.
+    if (!DS().ev_chi) CU(cudaEventCreateWithFlags(&DS().ev_chi, cudaEventDisableTiming));
     if (total > DS().chi_bytes) {
         if (DS().d_chi) {
-            CU(cudaStreamSynchronize(ctx.stream));
+            if (DS().chi_busy) CU(cudaEventSynchronize(DS().ev_chi));
             cudaFree(DS().d_chi);
             DS().d_chi = nullptr;
             DS().chi_bytes = 0;
+            DS().chi_busy = false;
         }
         CU(cudaMalloc(&DS().d_chi, total));
         DS().chi_bytes = total;
+    }
+    if (DS().chi_busy && DS().chi_stream != s) CU(cudaStreamWaitEvent(s, DS().ev_chi, 0));
+    if (nlens > lh::LAUNCH_RECORDS) {
+        const size_t big = npix > (size_t)K ? npix : (size_t)K;
+        if ((rc = ensure_carry((size_t)5 * big * sizeof(double), s))) return rc;
+    }
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    {
+        cudaError_t terr;
+        if (!device_math_tables(dev, &terr)) return fail(LH_ECUDA, "math tables: %s", cudaGetErrorString(terr));
     }
     char *B = DS().d_chi;
     double *ax = reinterpret_cast<double *>(B + o_ax), *ay = reinterpret_cast<double *>(B + o_ay);
@@ -503,10 +556,8 @@ int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constra
     double *src = sources ? sources : reinterpret_cast<double *>(B + o_src);
     unsigned long long *cnt = reinterpret_cast<unsigned long long *>(B + o_cnt);
     lh_image *im = reinterpret_cast<lh_image *>(B + o_im);
-    cudaStream_t s = ctx.stream;
-    int dev = 0, sms = 0;
-    CU(cudaGetDevice(&dev));
-    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    EvalOpts packed;
+    packed.packed0 = 0;
 
     // stage 2: unlens the constraints at their own positions, barycentre per source
     if (K > 0) {
@@ -515,7 +566,7 @@ int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constra
         ++ctx.launches;
         lh_grid pg = {0.0, 0.0, 1.0, K, 1};
         double *po[NPLANES] = {bax, bay, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-        EvalOpts opt;
+        EvalOpts opt = packed;
         opt.px = cx; opt.py = cy;
         if ((rc = eval_device(lenses, 1, nlens, &pg, po, opt))) return rc;
     }
@@ -523,13 +574,16 @@ int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constra
     ++ctx.launches;
     // stage 1: deflection on the grid
     double *go[NPLANES] = {ax, ay, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    if ((rc = eval_device(lenses, 1, nlens, g, go))) return rc;
+    if ((rc = eval_device(lenses, 1, nlens, g, go, packed))) return rc;
     // stage 3: predicted images
     CU(cudaMemsetAsync(cnt, 0, sizeof(*cnt), s));
     CU(lh::launch_delens_dev(ax, ay, g->x0, g->y0, g->dx, g->nx, g->ny, src, N, im, cap, cnt, sms, s, &ctx.launches));
     // stage 4: closest image of the same source, chi^2
     CU(lh::launch_assign_and_sum(dc, K, im, cnt, cap, predicted, term, chi2, nimages, s));
     ctx.launches += (K > 0) + 1;
+    CU(cudaEventRecord(DS().ev_chi, s));
+    DS().chi_busy = true;
+    DS().chi_stream = s;
     return LH_OK;
 }
 
@@ -543,6 +597,9 @@ int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_gri
     int nreq = 0;
     for (int k = 0; k < NPLANES; ++k) nreq += hp[k] != nullptr;
     if (!nreq) return fail(LH_EINVAL, "no output plane requested");
+    // validate and pack every model ONCE, before anything is enqueued or copied (LH_EINVAL: nothing written); the
+    // pieces below reuse the packed table
+    if ((rc = pack_all(lenses, nmodel, nlens))) return rc;
     const size_t plane_bytes = (size_t)nmodel * g->nx * g->ny * sizeof(double);
     const size_t need = plane_bytes * nreq;
     if (need > DS().planes_bytes) {
@@ -580,12 +637,12 @@ int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_gri
         const size_t count = nmodel == 1 ? (size_t)nu * g->nx : (size_t)nu * npix;
         for (int k = 0; k < NPLANES; ++k) sub[k] = dp[k] ? dp[k] + off : nullptr;
         EvalOpts opt;
-        if (nmodel == 1) { opt.j0 = u0; opt.nrows = nu; }
-        rc = nmodel == 1 ? eval_device(lenses, 1, nlens, g, sub, opt)
-                         : eval_device(lenses + (size_t)u0 * nlens, nu, nlens, g, sub);
-        if (rc) {
+        if (nmodel == 1) { opt.j0 = u0; opt.nrows = nu; opt.packed0 = 0; }
+        else opt.packed0 = u0;
+        rc = eval_device(lenses, nmodel == 1 ? 1 : nu, nlens, g, sub, opt);
+        if (rc) {  // only a CUDA failure can get here: the lens lists were validated above
             cudaStreamSynchronize(DS().copy_stream);
-            return rc;  // a lens was rejected on the first piece: nothing enqueued, nothing written
+            return rc;
         }
         CU(cudaEventRecord(DS().ev_piece[piece], ctx.stream));
         CU(cudaStreamWaitEvent(DS().copy_stream, DS().ev_piece[piece], 0));
@@ -666,38 +723,6 @@ int lh_math_host_eval(int fn, const double *a, const double *b, size_t n, double
             default: lh::rcp4(a[k], b[k], a[k] + b[k], 2.0 * b[k], i1, i2, i3, i4); out[k] = i1; break;
         }
     }
-    return LH_OK;
-}
-
-int lh_fp64_issue_probe(int variant, int extra, int warps_per_subpartition, int iters, double *cycles_per_group) {
-    ctx.err[0] = 0;
-    if (iters <= 0 || !cycles_per_group || warps_per_subpartition < 1 || warps_per_subpartition > 16)
-        return fail(LH_EINVAL, "lh_fp64_issue_probe: bad argument");
-    int dev = 0, sms = 0, khz = 0;
-    CU(cudaGetDevice(&dev));
-    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CU(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev));
-    if (!DS().d_sink) CU(cudaMalloc(&DS().d_sink, 64));
-    const int blocks = sms * warps_per_subpartition;  // 128 threads = one warp per sub-partition per block
-    cudaEvent_t t0, t1;
-    CU(cudaEventCreate(&t0));
-    CU(cudaEventCreate(&t1));
-    cudaError_t e = lh::launch_issue_probe(variant, extra, iters / 8 + 1, blocks, DS().d_sink, ctx.stream);  // warm-up
-    if (e == cudaErrorInvalidValue) {
-        cudaGetLastError();
-        return fail(LH_EINVAL, "lh_fp64_issue_probe: unknown variant %d / extra %d", variant, extra);
-    }
-    CU(e);
-    CU(cudaEventRecord(t0, ctx.stream));
-    CU(lh::launch_issue_probe(variant, extra, iters, blocks, DS().d_sink, ctx.stream));
-    CU(cudaEventRecord(t1, ctx.stream));
-    CU(cudaEventSynchronize(t1));
-    ctx.launches += 2;
-    float ms = 0.f;
-    CU(cudaEventElapsedTime(&ms, t0, t1));
-    cudaEventDestroy(t0);
-    cudaEventDestroy(t1);
-    *cycles_per_group = (double)ms * 1e-3 * (double)khz * 1e3 / ((double)iters * warps_per_subpartition);
     return LH_OK;
 }
 

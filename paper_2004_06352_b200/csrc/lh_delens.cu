@@ -9,8 +9,9 @@
 // One thread owns one grid cell (two triangles, cut along V10-V01).  The sources of a launch
 // travel in the kernel parameters, so the source index is warp-uniform and each source reaches the
 // comparisons as a uniform operand; a cell first rejects a source against the bounding box of its
-// four source-plane corners (the common, convergent path) and only then runs the exact barycentric
-// test.  The test arithmetic is written with the round-to-nearest intrinsics, i.e. WITHOUT FMA
+// four source-plane corners (the common, convergent path: that box contains the boxes of both
+// triangles, so nothing the definition accepts is lost) and only then runs, per triangle, the
+// definition of R22: closed bounding box of the three vertices AND the barycentric test.  The test arithmetic is written with the round-to-nearest intrinsics, i.e. WITHOUT FMA
 // contraction: it takes an integer decision (inside / outside) and must take it in exactly the
 // arithmetic the definition states, so that a triangle id never depends on the compiler.
 // Found images are appended through one atomic counter (order is not defined).
@@ -45,6 +46,10 @@ __device__ __forceinline__ double cross_rn(double ax, double ay, double bx, doub
 
 __device__ __forceinline__ void test_triangle(const DelensParams &P, int s, double sx, double sy, const double (&T)[4][2],
                                               const double (&B)[4][2], int a, int b, int c, long long tri) {
+    // R22: inside = inside the closed bounding box of the triangle's three vertices AND the barycentric test
+    if (sx < fmin(fmin(B[a][0], B[b][0]), B[c][0]) || sx > fmax(fmax(B[a][0], B[b][0]), B[c][0]) ||
+        sy < fmin(fmin(B[a][1], B[b][1]), B[c][1]) || sy > fmax(fmax(B[a][1], B[b][1]), B[c][1]))
+        return;
     const double e1x = __dsub_rn(B[b][0], B[a][0]), e1y = __dsub_rn(B[b][1], B[a][1]);
     const double e2x = __dsub_rn(B[c][0], B[a][0]), e2y = __dsub_rn(B[c][1], B[a][1]);
     const double px = __dsub_rn(sx, B[a][0]), py = __dsub_rn(sy, B[a][1]);
@@ -86,7 +91,7 @@ __global__ void __launch_bounds__(DELENS_THREADS) delens_kernel(const __grid_con
         for (int s = 0; s < P.nsources; ++s) {
             const double sx = DEV_SRC ? __ldg(P.dsrc + 2 * s) : P.src[s][0];
             const double sy = DEV_SRC ? __ldg(P.dsrc + 2 * s + 1) : P.src[s][1];
-            // a point of a closed triangle lies inside the bounding box of its vertices: exact reject
+            // outside the box of the four corners = outside the box of either triangle (R22): reject
             if (sx < lox || sx > hix || sy < loy || sy > hiy) continue;
             test_triangle(P, s, sx, sy, T, B, 0, 1, 2, 2 * cell);
             test_triangle(P, s, sx, sy, T, B, 3, 2, 1, 2 * cell + 1);

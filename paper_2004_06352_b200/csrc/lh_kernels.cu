@@ -1,9 +1,10 @@
 // lh_kernels.cu -- the pixel x lens superposition kernel (steps a2-a6).
 //
 // One thread owns PX horizontally adjacent pixels and keeps their accumulators in
-// registers; a CTA owns a TILE_W x TILE_H pixel tile; the lens table of the model is
-// streamed through shared memory in tiles of TL records and every warp reads the same
-// record at the same time (broadcast 128-bit LDS, no bank conflicts).  FP64 throughout.
+// registers; a CTA owns a TILE_W x TILE_H pixel tile.  The lens records of a launch travel
+// BY VALUE in the kernel parameters (constant bank 0) and reach the FP64 instructions as
+// uniform-register operands (LDCU), one field per instruction; only the atan / atanh
+// reduction tables are staged in shared memory.  FP64 throughout.
 //
 // Accumulators per pixel:  ax, ay  (eq. 10)
 //                          S = a11+a22, Dl = a11-a22, a12   (sec. 2.4)
@@ -58,10 +59,10 @@ using SmemTables = MathTables;  // the atan / atanh reduction tables, staged per
 //   alpha'_x = G atan ( x' (P^_t - P^_c) / (P^_c P^_t + x'^2) )
 //   alpha'_y = G atanh( y' (Q^_t - Q^_c) / (Q^_c Q^_t - y'^2) ),         G = T k
 //   D_r = (sg^2/p) (P^_r^2 + x'^2),  f^_r = 1 / (w^_r (P^_r^2 + x'^2)) = f_r / (k p / sg^2)
-//   a11 + a22 += G  (1/w^_c - 1/w^_t)
+//   a11 + a22 += G  (1/w^_c - 1/w^_t),   1/w^_r = f^_r (P^_r^2 + x'^2)
 //   a11 - a22 += TF [ K (f^_c rc^2 - f^_t rt^2) - (dx^2 - dy^2)(f^_c - f^_t) ],  K  = -4 eps cos 2theta
 //   a12       += TF [ K'(f^_c rc^2 - f^_t rt^2) -  dx dy       (f^_c - f^_t) ],  K' = -2 eps sin 2theta
-// The four reciprocals (reduced atan / atanh denominators, D^_c, D^_t) come from ONE seed (rcp4).
+// The four reciprocals (reduced atan / atanh denominators, w^_c D^_c, w^_t D^_t) come from ONE seed (rcp4).
 // RULE: no FP64 instruction may take TWO lens fields.  One of them would have to be copied into a
 // vector register, and ptxas then gives up the uniform datapath for the whole record (vector LDC,
 // 3-register FMAs everywhere) -- measured, and guarded by tests/test_sass_cpu.py.
@@ -72,12 +73,11 @@ __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Ac
     const double yp = fma(-L.s, dx, L.c * dy);
     const double xx = xp * xp, yy = yp * yp;
     const double vc = fma(L.ip, xx, L.im * yy) + L.rc2;  // k^2 (rc^2 + rho^2)
-    double wc, iwc, wt, iwt;
-    rsqrt_sqrt(vc, wc, iwc);
-    rsqrt_sqrt(vc + L.dr2, wt, iwt);  // k^2 (rt^2 + rho^2)
+    const double wc = sqrt_pos(vc);
+    const double wt = sqrt_pos(vc + L.dr2);  // k^2 (rt^2 + rho^2)
     const double Pc = wc + L.ac, Pt = wt + L.at;
     Reduced ra, rh;
-    double Dc = 1.0, Dt = 1.0, i1, i2, i3, i4;
+    double Dc = 1.0, Dt = 1.0, i1, i2, fc, ft;
     if (GRAD) {
         // P^_t > P^_c and Q^_t > Q^_c (rcut > rcore): the arguments carry the signs of x' and y'
         const double Qc = wc + L.bc, Qt = wt + L.bt;
@@ -88,12 +88,13 @@ __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Ac
         Dc = fma(Pc, Pc, xx);
         Dt = fma(Pt, Pt, xx);
     }
+    // f^_r = 1/(w^_r D_r) straight from the shared reciprocal; 1/w^_r is then f^_r D_r
     if (GRAD && HESS)
-        rcp4(ra.den, rh.den, Dc, Dt, i1, i2, i3, i4);
+        rcp4(ra.den, rh.den, wc * Dc, wt * Dt, i1, i2, fc, ft);
     else if (GRAD)
         rcp2(ra.den, rh.den, i1, i2);
     else
-        rcp2(Dc, Dt, i3, i4);
+        rcp2(wc * Dc, wt * Dt, fc, ft);
     if (GRAD) {
         const double at = atan_finish(ra, i1, xp);
         const double ah = atanh_finish(rh, i2, yp);
@@ -101,10 +102,9 @@ __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Ac
         a.ay = fma(L.sG, at, fma(L.cG, ah, a.ay));
     }
     if (HESS) {
-        const double fc = iwc * i3, ft = iwt * i4;
         const double u = fma(fc, L.r2c, -(ft * L.r2t));
         const double Tv = L.TF * (fc - ft);
-        a.S = fma(L.G, iwc - iwt, a.S);
+        a.S = fma(L.G, fma(fc, Dc, -(ft * Dt)), a.S);
         a.Dl = fma(L.KTF, u, fma(-fma(dx, dx, -(dy * dy)), Tv, a.Dl));
         a.a12 = fma(L.K2TF, u, fma(-(dx * dy), Tv, a.a12));
     }
@@ -141,7 +141,7 @@ __device__ __forceinline__ void nsie_term(const LensK &L, double X, double Y, Ac
     }
 }
 
-// ---- CLS_EXTREME: dPIE / NSIE with eps > EXTREME_EPS (axis ratio < 0.02) ----------------------
+// ---- CLS_EXTREME: dPIE / NSIE with eps > EXTREME_EPS (axis ratio < 0.081) ---------------------
 // Rare and slow on purpose: the two PIEMD terms are evaluated one by one (same
 // scaled frame) with IEEE sqrt / division and libdevice atan / atanh -- no table range limits, no
 // merged-form cancellation in Q^_c Q^_t - y'^2 as the atanh argument -> 1.  L.rt2 == 0 marks an
@@ -215,7 +215,7 @@ __device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc
 // (LDCU) into a uniform register and enters the FP64 instructions as their one uniform
 // operand.  That matters because the B200 FP64 pipe issues a warp instruction every 2 cycles
 // only while it reads at most two distinct vector registers; an FMA with three costs 3
-// (profiles/r01_fp64_operand_probe.md).  A record staged in shared memory would land in
+// (profiles/r01_fp64_issue_probes.md).  A record staged in shared memory would land in
 // vector registers and make almost every FMA of the lens algebra a 3-register one.
 //
 // ptxas only moves the record fields to the uniform datapath (LDCU) when the vector register
@@ -246,7 +246,10 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
     // a2: pixel coordinates from the grid definition (no coordinate array in memory)
     // (in grid mode every Yk[k] is the same value, so the row-wise subexpressions of the lens algebra are shared)
     double X[PX], Yk[PX];
-    const double Y = fma((double)(j + P.j0), P.dx, P.y0);
+    // X_i = x0 + i dx, Y_j = y0 + j dx as TWO rounded operations (no FMA contraction): the same coordinate the
+    // delensing kernel gives the grid vertex (lh_delens.cu) and the definition states (include/lh.h), so that the
+    // deflection is evaluated at exactly the vertex the triangles are built on, also where dx is not dyadic
+    const double Y = __dadd_rn(P.y0, __dmul_rn((double)(j + P.j0), P.dx));
 #pragma unroll
     for (int k = 0; k < PX; ++k) {
         if (POINTS) {
@@ -254,7 +257,7 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
             X[k] = in ? __ldg(P.px + i0 + k) : 0.0;
             Yk[k] = in ? __ldg(P.py + i0 + k) : 0.0;
         } else {
-            X[k] = fma((double)(i0 + k), P.dx, P.x0);
+            X[k] = __dadd_rn(P.x0, __dmul_rn((double)(i0 + k), P.dx));
             Yk[k] = Y;
         }
     }
@@ -412,17 +415,18 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     bool hess = false;
     for (int k = 2; k < 9; ++k) hess = hess || J.out[k];
 
+    cudaStream_t cur = stream;  // stream the next launch goes to (`stream`, or J.aux for every other chunked model)
     auto go = [&](int nm, bool extreme) -> cudaError_t {
         dim3 grid((unsigned)tiles, (unsigned)nm, 1);
         ++*launches;
         if (extreme) {
-            if (grad && hess) return launch_one<true, true, true>(Q, grid, stream);
-            if (grad) return launch_one<true, false, true>(Q, grid, stream);
-            return launch_one<false, true, true>(Q, grid, stream);
+            if (grad && hess) return launch_one<true, true, true>(Q, grid, cur);
+            if (grad) return launch_one<true, false, true>(Q, grid, cur);
+            return launch_one<false, true, true>(Q, grid, cur);
         }
-        if (grad && hess) return launch_one<true, true, false>(Q, grid, stream);
-        if (grad) return launch_one<true, false, false>(Q, grid, stream);
-        return launch_one<false, true, false>(Q, grid, stream);
+        if (grad && hess) return launch_one<true, true, false>(Q, grid, cur);
+        if (grad) return launch_one<true, false, false>(Q, grid, cur);
+        return launch_one<false, true, false>(Q, grid, cur);
     };
 
     const int n = J.nlens;
@@ -472,13 +476,31 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
         }
         return cudaSuccess;
     }
-    // one model at a time, balanced lens chunks
-    for (int m = 0; m < J.nmodel; ++m) {
-        cudaError_t e = chunks(J.table + (size_t)m * n, J.ranges[m], n, m, true, true,
-                               J.stats ? ((m == J.nmodel - 1) ? 2 : 1) : 0);
-        if (e != cudaSuccess) return e;
+    // one model at a time, balanced lens chunks.  The chunks of ONE model depend on each other through `carry`;
+    // different models do not.  With a second stream and a second carry buffer the even and the odd models form two
+    // independent chains, so the partial last wave of one chain's launch is filled by the other chain's CTAs
+    // (cfg 4: 4096 CTAs over 888 resident slots = 4.6 waves per launch).  Statistics mode folds the models in order
+    // and stays on one stream.
+    const bool two = J.aux != nullptr && J.carry2 != nullptr && J.nmodel > 1 && !J.stats;
+    cudaError_t e = cudaSuccess;
+    if (two) {
+        if ((e = cudaEventRecord(J.ev_fork, stream)) != cudaSuccess) return e;
+        if ((e = cudaStreamWaitEvent(J.aux, J.ev_fork, 0)) != cudaSuccess) return e;
     }
-    return cudaSuccess;
+    for (int m = 0; m < J.nmodel && e == cudaSuccess; ++m) {
+        const bool odd = two && (m & 1);
+        cur = odd ? J.aux : stream;
+        Q.carry = odd ? J.carry2 : J.carry;
+        e = chunks(J.table + (size_t)m * n, J.ranges[m], n, m, true, true, J.stats ? ((m == J.nmodel - 1) ? 2 : 1) : 0);
+    }
+    cur = stream;
+    Q.carry = J.carry;
+    if (two) {  // join even after an error: `stream` must not run ahead of work already enqueued on the second stream
+        cudaError_t e2 = cudaEventRecord(J.ev_join, J.aux);
+        if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(stream, J.ev_join, 0);
+        if (e == cudaSuccess) e = e2;
+    }
+    return e;
 }
 
 // ---- FP64 roofline probe: independent DFMA chains, all SMs, full occupancy -------------------

@@ -8,7 +8,7 @@
 namespace lh {
 
 // Records one launch carries in its kernel parameters (constant bank 0, 32 764 bytes at most):
-// 160 x 192 B of lens constants + 160 x 8 B of class boundaries + a 152-byte header.
+// 160 x 192 B of lens constants + 160 x 8 B of class boundaries + a header of about 250 bytes.
 constexpr int LAUNCH_RECORDS = 160;
 constexpr int LAUNCH_MODELS = 160;  // models that may share one launch (blockIdx.y)
 
@@ -52,12 +52,16 @@ struct EvalJob {
     double *m2[9];   // DEVICE, stats only (else all nullptr)
     int stats;       // 0 = per-model planes [nmodel][ny][nx]; 1 = mean / variance over the models, planes [ny][nx]
     double *carry;   // DEVICE, 5*nx*ny doubles; needed only when nlens > LAUNCH_RECORDS
+    // optional second chain for batches of chunked models (all four or none): every other model runs on `aux` with
+    // `carry2`; launch_eval forks `aux` from the job's stream (ev_fork) and joins it back (ev_join) before returning
+    double *carry2 = nullptr;
+    cudaStream_t aux = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
 // Enqueues every launch of the job on `stream`; adds the number of kernels launched to *launches.
 cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launches);
 cudaError_t launch_dfma_probe(int iters, int blocks, double *sink, cudaStream_t stream);
-cudaError_t launch_issue_probe(int variant, int extra, int iters, int blocks, double *sink, cudaStream_t stream);  // lh_probe.cu
 
 // lh_delens.cu (NEXT row f1)
 cudaError_t launch_source_plane(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,

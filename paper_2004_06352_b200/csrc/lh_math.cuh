@@ -13,7 +13,9 @@
 //      good to a few ulp.  Several reciprocals share one seed and one correction through
 //      the reciprocal of their product (rcp2 / rcp4).
 //   3. for atan / atanh: range reduction against a shared-memory table indexed by the
-//      exponent and the top 6 mantissa bits of the approximate quotient (seed x numerator),
+//      exponent and the top 6 mantissa bits of the approximate quotient (seed x numerator;
+//      the additive constants of the two index arguments ride in the FMA that forms them, so
+//      that each index costs shift + biased unsigned min + address + LDS and nothing else),
 //      with the quotient folded into the reduced argument so that each function needs ONE
 //      refined reciprocal:
 //        atan(n/d)  = atan(c) + atan( (|n| - c d)/(d + c |n|) ),  c = |n|/d rounded to 6 bits
@@ -37,8 +39,11 @@
 
 namespace lh {
 
-// Both tables: entry 0 is the identity (c = 0 / c' = 0), entry 1 + 64 o + k is
-// c = 2^(o + O_MIN) (1 + k/64).
+// atan table, indexed by the exponent / 6-mantissa-bit code of q' = q + 2^-8 (q = |n|/d approximately):
+//   entry 0                      q' in [2^-8, 2^-8 (1 + 1/64))  i.e. q < 2^-14: the identity, c = 0
+//   entry 64 o + k (1..1023)     q' in 2^(o-8) [1 + k/64, 1 + (k+1)/64):  c = 2^(o-8) (1 + (k + 1/2)/64) - 2^-8
+//   entry 1024                   q' >= 2^8:  c = 2^8  (z = (q - c)/(1 + c q) stays below 1/c)
+// atanh table: entry 0 is the identity (c' = 0); see quot_index_down.
 constexpr int TAB_PER_OCT = 64;
 constexpr int ATAN_OCT_MIN = -8, ATAN_OCTAVES = 16;  // quotient in [2^-8, 2^8)
 constexpr int ATAN_N = ATAN_OCTAVES * TAB_PER_OCT + 1;
@@ -104,7 +109,7 @@ LH_HD void rcp2(double a, double b, double &ia, double &ib) {
 }
 
 // four reciprocals from one seed (product tree).                      12 FP64 + 1 MUFU
-// The product a b c d must stay inside the double range: lengths within ~1e+-35 (lh.h).
+// The product a b c d must stay inside the double range (lh.h states the resulting range of lengths).
 LH_HD void rcp4(double a, double b, double c, double d, double &ia, double &ib, double &ic, double &id) {
     const double ab = a * b, cd = c * d;
     const double r = rcp(ab * cd);
@@ -128,31 +133,41 @@ LH_HD void rsqrt_sqrt(double v, double &w, double &iw) {
     w = fma(t, h, t);
 }
 
+// w = sqrt(v) alone (same seed and step as rsqrt_sqrt, without the closing FMA of 1/sqrt).   5 FP64 + 1 MUFU
+LH_HD double sqrt_pos(double v) {
+    const double y = rsq_seed(v);
+    const double t = v * y;
+    const double e = fma(-t, y, 1.0);
+    const double h = fma(0.375, e, 0.5) * e;
+    return fma(t, h, t);
+}
+
 // copysign as ONE integer operation on the high word (1 dispatch cycle, not 2); mag >= 0
 LH_HD double copysign_pos_i(double mag, double sgn) { return mk64(hi32(mag) | (hi32(sgn) & (int)0x80000000), lo32(mag)); }
 
-// Table index of a positive quotient q (approximate is enough): exponent and top 6 mantissa
-// bits, rounded to nearest; `bias` is the exponent of entry 1.  Everything below the table maps
-// to entry 0 (the identity), everything above (and NaN patterns) to the last entry.
-LH_HD unsigned quot_index(double q, int oct_min, int n) {
-    const int hr = hi32(q) + 0x2000;  // round to 6 mantissa bits (bit 13 is half a step)
-    const int j = (hr >> 14) - ((1023 + oct_min) << 6) + 1;
+// Table index of q' = q + 2^-8 >= 2^-8 (q >= 0 approximate quotient): exponent and top 6 mantissa bits,
+// truncated, counted from the code of 2^-8.  No lower clamp is needed (q' >= 2^-8 by construction); the
+// unsigned min sends everything at or above 2^8 -- and NaN / negative garbage -- to the last entry.
+LH_HD unsigned quot_index_up(double qp, int n) {
+    const unsigned j = (unsigned)((hi32(qp) >> 14) - ((1023 + ATAN_OCT_MIN) << 6));
 #ifdef __CUDA_ARCH__
-    return min((unsigned)max(j, 0), (unsigned)(n - 1));
+    return min(j, (unsigned)(n - 1));
 #else
-    return (unsigned)(j < 0 ? 0 : (j > n - 1 ? n - 1 : j));
+    return j > (unsigned)(n - 1) ? (unsigned)(n - 1) : j;
 #endif
 }
 
 // Table index of t in (0, 1] counted DOWN from 1: entry 0 is t = 1 (c' = 0), entry 64 o + k,
-// k = 0..63, is t_c = 2^-(o+1) (2 - k/64) ... i.e. the exponent/6-bit-mantissa code of t
-// subtracted from that of 1.0.  t above 1 (rounding) maps to entry 0, t below the table to the last.
+// k = 0..63, is t_c = 2^-(o+1) (2 - k/64) ... i.e. the exponent/6-bit-mantissa code of t, rounded to
+// nearest, subtracted from that of 1.0.  The caller guarantees t <= 1 (atanh_reduce forms it as
+// 1 - an * seed), so the difference is never negative; t below the table -- and NaN / negative garbage,
+// whose difference wraps to a large unsigned -- maps to the last entry.
 LH_HD unsigned quot_index_down(double t, int n) {
-    const int j = ((1023 << 20) + 0x2000 - hi32(t)) >> 14;  // round((code(1.0) - code(t)) / 2^14)
+    const unsigned j = (unsigned)(((1023 << 20) + 0x2000 - hi32(t))) >> 14;  // round((code(1.0) - code(t)) / 2^14)
 #ifdef __CUDA_ARCH__
-    return min((unsigned)max(j, 0), (unsigned)(n - 1));
+    return min(j, (unsigned)(n - 1));
 #else
-    return (unsigned)(j < 0 ? 0 : (j > n - 1 ? n - 1 : j));
+    return j > (unsigned)(n - 1) ? (unsigned)(n - 1) : j;
 #endif
 }
 
@@ -166,8 +181,8 @@ struct Reduced {
     double num, den, base;
 };
 LH_HD Reduced atan_reduce(double an, double d, const double2 *__restrict__ tab) {
-    const double q0 = an * rcp_seed(d);  // |n|/d to 1e-6
-    const double2 ca = tab[quot_index(q0, ATAN_OCT_MIN, ATAN_N)];
+    const double qp = fma(an, rcp_seed(d), 0x1p-8);  // |n|/d to 1e-6, + 2^-8: the index needs no lower clamp
+    const double2 ca = tab[quot_index_up(qp, ATAN_N)];
     return Reduced{fma(-ca.x, d, an), fma(ca.x, an, d), ca.y};
 }
 LH_HD double atan_finish(const Reduced &r, double iden, double sgn) {
@@ -185,9 +200,11 @@ LH_HD double atan_finish(const Reduced &r, double iden, double sgn) {
 // Both FMAs see the exact an and d.  The host packer (lh_pack.cpp) routes every lens whose
 // ellipticity could push u past the table into the CLS_EXTREME class, which does not come
 // through here; the index is clamped all the same.
-//   atanh_reduce  4 FP64 + 1 MUFU      atanh_finish  5 FP64
+// t is formed as 1 - an * seed(d) (one FMA): its ABSOLUTE error is u * 2^-19.9, which against the bin
+// half-width t/128 is negligible as long as t > 2^-8.6, i.e. eps <= EXTREME_EPS = 0.85 (lh_pack.h).
+//   atanh_reduce  3 FP64 + 1 MUFU      atanh_finish  5 FP64
 LH_HD Reduced atanh_reduce(double an, double d, const double2 *__restrict__ tab) {
-    const double t0 = (d - an) * rcp_seed(d);  // 1 - u to 1e-6 relative
+    const double t0 = fma(-an, rcp_seed(d), 1.0);  // 1 - u, absolute error u 2^-19.9; never above 1
     const double2 ca = tab[quot_index_down(t0, LN_N)];
     return Reduced{fma(-ca.x, d, an), fma(-ca.x, an, d), ca.y};
 }
@@ -211,10 +228,14 @@ LH_HD double atanh_nd(double n, double d, const double2 *__restrict__ tab) {
 // host: fill the tables (long-double libm: they are constants of the library)
 inline void fill_math_tables(MathTables &T) {
     T.at[0] = make_double2(0.0, 0.0);
-    for (int j = 1; j < ATAN_N; ++j) {
-        const int e = (j - 1) / TAB_PER_OCT + ATAN_OCT_MIN, m = (j - 1) % TAB_PER_OCT;
-        const double c = std::ldexp(1.0 + (double)m / TAB_PER_OCT, e);
+    for (int j = 1; j < ATAN_N - 1; ++j) {
+        const int e = j / TAB_PER_OCT + ATAN_OCT_MIN, m = j % TAB_PER_OCT;
+        const double c = std::ldexp(1.0 + ((double)m + 0.5) / TAB_PER_OCT, e) - std::ldexp(1.0, ATAN_OCT_MIN);  // exact
         T.at[j] = make_double2(c, (double)atanl((long double)c));
+    }
+    {
+        const double c = std::ldexp(1.0, ATAN_OCT_MIN + ATAN_OCTAVES);
+        T.at[ATAN_N - 1] = make_double2(c, (double)atanl((long double)c));
     }
     // entry j <-> code(1.0) - j: j = 64 o + k, k = 1..64  ->  t_c = 2^-(o+1) (2 - k/64)  (k = 64: 2^-(o+1))
     for (int j = 0; j < LN_N; ++j) {

@@ -24,6 +24,7 @@ static int classify(const lh_lens &L, int idx, int model, char *err, int errlen)
     if (L.type == LH_SIS) {
         // ellipticity, theta, rcore, rcut are ignored for an SIS (reading 8c-19) -- only what is used must be finite
         if (!(std::isfinite(L.x) && std::isfinite(L.y) && std::isfinite(L.b0))) return fail("non-finite parameter");
+        if (!(L.b0 >= 0.0)) return fail("b0 must be >= 0");
         return CLS_SIS;
     }
     if (L.type == LH_NSIE) {
@@ -33,6 +34,7 @@ static int classify(const lh_lens &L, int idx, int model, char *err, int errlen)
     } else if (!finite_all(L)) {
         return fail("non-finite parameter");
     }
+    if (!(L.b0 >= 0.0)) return fail("b0 must be >= 0");
     if (!(L.ellipticity >= 0.0 && L.ellipticity < 1.0)) return fail("ellipticity outside [0,1)");
     if (!(L.rcore > 0.0)) return fail("rcore must be > 0");
     if (L.type == LH_DPIE && !(L.rcut > L.rcore)) return fail("dPIE needs rcut > rcore");
@@ -57,10 +59,10 @@ static void fill(const lh_lens &L, int cls, LensK &K) {
     const bool cut = (L.type == LH_DPIE);
     const double rt = cut ? L.rcut : 0.0;
     const double T = cut ? L.b0 * rt / (rt - rc) : L.b0;
-    // eps -> 0 is taken by never letting 2 sqrt(eps) fall below 2^-64: the scaled frame then makes x'^2
+    // eps -> 0 is taken by never letting 2 sqrt(eps) fall below 2^-40: the scaled frame then makes x'^2
     // vanish against P^_c P^_t exactly (atan(u) = u below 1e-8) and every product stays far inside the
-    // double range; the deviation from the true tiny eps is O(eps) < 2^-130 relative.
-    const double sg = std::fmax(2.0 * std::sqrt(eps), 0x1p-64);
+    // double range; the deviation from the true tiny eps is O(2^-82) relative.
+    const double sg = std::fmax(2.0 * std::sqrt(eps), 0x1p-40);
     const double k = o / sg;
     const double c2 = std::cos(2.0 * L.theta), s2 = std::sin(2.0 * L.theta);
     K.c = std::cos(L.theta);

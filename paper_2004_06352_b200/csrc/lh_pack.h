@@ -4,8 +4,9 @@
 // lens, the constants that do not depend on the pixel.  PAPER.md:151 (sec. 3.2.1)
 // argues for SoA so that SIMD lanes over *lenses* load homogeneous data; on the
 // GPU the lanes run over *pixels* and every lane of a warp needs the same lens at
-// the same time, so the right layout is one contiguous, 16-byte aligned record
-// per lens that a warp fetches from shared memory as broadcast 128-bit loads.
+// the same time, so the right layout is one contiguous record per lens.  The records of
+// a launch travel BY VALUE in the kernel parameters (constant bank 0, lh_kernels.h) and
+// reach the FP64 instructions as uniform-register operands (LDCU), one field each.
 #pragma once
 #include <cstdint>
 
@@ -21,12 +22,14 @@ enum LensClass : int {
     CLS_COUNT = 4
 };
 
-// Above this eps = (1-q)/(1+q) the ratio (1+u)/(1-u), u = 2 sqrt(eps)/(1+eps), approaches the 2^16 end
-// of the atanh table: eps = 0.96 <-> e-hat = 0.99917 <-> axis ratio q = 0.0204 <-> ratio < 9700.
-constexpr double EXTREME_EPS = 0.96;
+// Above this eps = (1-q)/(1+q) the atanh argument u = 2 sqrt(eps)/(1+eps) comes so close to 1 that the fast
+// atanh's index argument t = 1 - u, formed with an ABSOLUTE error of u 2^-19.9 (lh_math.cuh), is no longer
+// good to a small fraction of its bin: eps = 0.85 <-> e-hat = 0.987 <-> axis ratio q = 0.081 <-> t >= 3.3e-3
+// (index error < 3 % of the bin half-width); the table itself would reach to t = 2^-16.
+constexpr double EXTREME_EPS = 0.85;
 
 // Notation: eps = e/(1+sqrt(1-e^2)), o = 1-eps^2, p = (1+eps)^2, m = (1-eps)^2,
-// sg = 2 sqrt(eps) (never below 2^-64, which takes the circular limit), k = o/sg,
+// sg = 2 sqrt(eps) (never below 2^-40, which takes the circular limit), k = o/sg,
 // T = b0*rt/(rt-rc) (dPIE) or b0 (NSIE, SIS), c/s = cos/sin(theta).
 // All lengths of the lens frame are carried scaled by k (w^ = k w), which removes the
 // 2 sqrt(eps) factors from the atan / atanh arguments (sec. 5.2) and turns D_r into

@@ -86,3 +86,36 @@ def test_chi2_argument_errors():
         lh.lh_chi2(badlens, g, li.make_constraints([(0, 0.0, 0.0, 1.0)]), 1, chi)
     torch.cuda.synchronize()
     assert torch.isnan(chi).all()
+
+
+def test_chi2_on_two_streams_does_not_share_scratch_unsafely():
+    """lh_chi2 keeps its scratch (deflection planes, sources, image list, counter) in ONE cached buffer per device.
+    Calls on different streams must not overwrite it while an earlier call is still running: the second stream waits
+    for the first call's end event.  Two different problems alternate on two streams, several times, each result is
+    compared with the result of the same call made alone."""
+    c = li.config(1, scale=4)
+    g = c.grid
+    cons_a, ns_a = _cluster_constraints(c, g, 40, seed=5)
+    cons_b, ns_b = _cluster_constraints(c, g, 30, seed=9)
+    Lb = c.lenses.copy()
+    Lb["b0"][0] *= 1.05
+    alone_a, alone_b = gpu_chi2(c.lenses, g, cons_a, ns_a), gpu_chi2(Lb, g, cons_b, ns_b)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    torch.cuda.synchronize()
+    try:
+        for k in range(4):
+            for st, (L, cons, ns) in ((s1, (c.lenses, cons_a, ns_a)), (s2, (Lb, cons_b, ns_b))):
+                chi = torch.full((1,), float("nan"), dtype=torch.float64, device="cuda")
+                pred = torch.full((len(cons), 2), 7.0, dtype=torch.float64, device="cuda")
+                nim = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+                lh.lh_set_stream(st)
+                lh.lh_chi2(L, g, cons, ns, chi, pred, None, nim)
+                outs.append((chi, pred, nim))
+    finally:
+        lh.lh_set_stream(None)
+    torch.cuda.synchronize()
+    for k, (chi, pred, nim) in enumerate(outs):
+        want = alone_a if k % 2 == 0 else alone_b
+        assert float(chi.item()) == want["chi2"] and int(nim.item()) == want["nimages"]
+        assert np.array_equal(pred.cpu().numpy(), want["predicted"])

@@ -179,7 +179,8 @@ def test_chunked_model_with_every_class():
 
 
 def test_extreme_length_scales_stay_inside_the_shared_reciprocal_range():
-    """rcp4 takes the reciprocal of a product of four squared lengths (include/lh.h: lengths within ~1e+-35):
+    """rcp4 takes the reciprocal of a product of two squared and two cubed scaled lengths (include/lh.h: lengths
+    between ~1e-20 and ~1e+17 of the unit in use):
     micro-arcsec and 1e12-arcsec units must still give oracle-grade results."""
     for scale in (1e-9, 1e12):
         L = li.make_lenses(2)
@@ -523,3 +524,38 @@ def test_host_entry_point_pipelined_pieces_are_bitwise_the_device_result():
 def test_fp64_probe_runs():
     flops, secs = lh.lh_fp64_peak_probe(2048)
     assert secs > 0 and 1e12 < flops < 1e14
+
+
+def test_host_entry_point_validates_every_model_before_writing_anything():
+    """A bad lens in the LAST model of a batch large enough to be pipelined in pieces (>= 8 MB of results): LH_EINVAL,
+    and not one element of the caller's host planes written (include/lh.h: nothing enqueued, nothing written)."""
+    c = li.config(4, scale=4)  # 64 models x 300 lenses on 256 x 256: 64 MB of results, 8 pieces
+    bad = c.lenses.copy()
+    bad["rcore"][-1] = -1.0
+    host = {n: np.full((c.nmodel, c.grid.ny, c.grid.nx), np.nan) for n in ("ax", "ay")}
+    n0 = lh.lh_launch_count()
+    with pytest.raises(lh.LhError) as e:
+        lh.lh_grid_eval_host(bad, c.nmodel, c.nlens, c.grid, **host)
+    assert e.value.code == lh.LH_EINVAL and "model 63" in str(e.value)
+    assert lh.lh_launch_count() == n0
+    assert all(np.isnan(v).all() for v in host.values())
+
+
+def test_binding_refuses_undersized_or_misplaced_tensors():
+    """The C ABI only sees addresses: the binding checks element counts (and the device) before the call."""
+    c = li.config(0)
+    g = c.grid
+    small = torch.empty(g.npix - 1, dtype=torch.float64, device="cuda")
+    ok = torch.empty(g.npix, dtype=torch.float64, device="cuda")
+    with pytest.raises(ValueError):
+        lh.lh_grid_gradient(c.lenses, g, small, ok)
+    with pytest.raises(ValueError):
+        lh.lh_grid_eval(c.lenses, g, kappa=small)
+    with pytest.raises(ValueError):
+        lh.lh_grid_gradient_batch(np.concatenate([c.lenses, c.lenses]), 2, c.nlens, g, ok, ok)  # needs 2 * npix
+    with pytest.raises(ValueError):
+        lh.lh_grid_eval_rows(c.lenses, g, 0, 3, ax=torch.empty(3 * g.nx - 1, dtype=torch.float64, device="cuda"))
+    with pytest.raises(ValueError):
+        lh.lh_grid_eval_host(c.lenses, 1, c.nlens, g, ax=np.empty(g.npix - 1))
+    with pytest.raises(TypeError):
+        lh.lh_grid_eval_host(c.lenses, 1, c.nlens, g, ax=ok)  # a device tensor where a host plane is expected
