@@ -1,19 +1,22 @@
 #!/usr/bin/env python
 """bench.py -- pixel-lens FP64 gradient+Hessian evaluations per second on B200.
 
-A "step" is one pass of the whole hot path (rows a1-a5: pack the lens
-list, hand the records to the launches, superpose first and second derivatives over all lenses at every
-pixel, fused kappa/gamma/mu epilogue, stores) over BASELINE.json config 3:
-4096 x 4096 pixels x 1000 dPIE potentials, outputs ax ay kappa gamma1 gamma2 mu, the
-Hessian never written.  One process per GPU; at N > 1 every rank evaluates its own lens
-model (an MCMC-style independent sample) on the same grid -- the path shards by
-independent problems with no exchange step, so there is no collective on the data path
-and `scaling` is "weak".
+A "step" is one pass of the whole hot path (rows a1-a5: pack the lens list, hand the records to
+the launches, superpose first and second derivatives over all lenses at every pixel, fused kappa/gamma/mu epilogue,
+stores) over BASELINE.json config 3: 4096 x 4096 pixels x 1000 dPIE potentials, outputs ax ay kappa gamma1 gamma2
+mu, the Hessian never written.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--scaling auto|strong|weak] [--impl reference]
 
-Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/) on the
-host cores on a bounded sample of the same workload.
+One process per GPU.  The path shards with no exchange step (pixels are independent):
+  * N > 1, --scaling strong (the default for N > 1, "the grid is split among the
+    GPUs", Fig. 7, Table A.4): rank r evaluates rows lens_inputs.row_slab(r, N) of the ONE map with lh_grid_eval_rows
+    on its own device, the whole lens list replicated; `value` = evals of the one map / the slowest rank's time.
+    Assembling the map on rank 0 (one gather of the slabs) is timed separately (`assemble`), it is not part of the
+    computation.
+  * --scaling weak: every rank evaluates its own lens model on the full grid (independent MCMC samples).
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded
+sample of the same workload.
 """
 from __future__ import annotations
 
@@ -28,42 +31,47 @@ import time
 import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
-if ROOT not in sys.path:
-    sys.path.insert(0, ROOT)
+for _p in (ROOT, os.path.join(ROOT, "tests")):
+    if _p not in sys.path:
+        sys.path.insert(0, _p)
 
 import lens_inputs as li  # noqa: E402
 
 METRIC = "pixel-lens FP64 gradient+Hessian evals/sec"
 UNIT = "evals/s"
 
-# Executed FP64 flops per (pixel, lens) dPIE evaluation of each kernel variant (2*DFMA + DMUL + DADD
-# thread-instructions / evaluations).  grad+hess: ncu counters, profiles/r01_cfg3_ncu.md (81.0 FP64
-# instructions, 120.0 flop); grad / hess: the same count read from the SASS inner loop (56.75 and 46
-# instructions).  DESIGN.md sec. 7.  This is what the hardware did -- `roofline.achieved` never claims more.
-FLOPS_PER_EVAL = {"grad+hess": 120.0, "grad": 84.75, "hess": 69.0}
-FP64_INSTR_PER_EVAL = {"grad+hess": 81.0, "grad": 56.75, "hess": 46.0}
+# Executed FP64 thread-instructions per (pixel, lens) dPIE evaluation of each kernel variant, (DFMA, DMUL, DADD), read
+# from the SASS of the lens loop of the built library: tests/test_sass_cpu.py RECOUNTS them with cuobjdump and fails
+# when these constants and the kernel drift apart (the loop holds PX = 4 evaluations).  flop = 2 DFMA + DMUL + DADD.
+# This is what the hardware did -- `roofline.achieved` never claims more.  DESIGN.md sec. 7.
+FP64_OPS_PER_EVAL = {"grad+hess": (40.0, 28.75, 10.25), "grad": (30.0, 16.5, 9.25), "hess": (22.0, 16.75, 6.25)}
+FP64_INSTR_PER_EVAL = {k: sum(v) for k, v in FP64_OPS_PER_EVAL.items()}
+FLOPS_PER_EVAL = {k: 2 * v[0] + v[1] + v[2] for k, v in FP64_OPS_PER_EVAL.items()}
 # SURVEY.md sec. 8(d) canonical count for the cheapest exact formulation it knew (context: this kernel's
 # formulation is cheaper, so evals/s x canonical flops can exceed the FLOP/s peak and is NOT a roofline fraction)
 CANONICAL_FLOPS_PER_EVAL = {"grad+hess": 278.0, "grad": 205.0, "hess": 105.0}
-# FP64 CUDA-core peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x SM clock (B200_PROFILING.md:
-# 148 SMs, clocks.max.sm 1965 MHz).  The live DFMA probe (lh_fp64_peak_probe) is the
-# measured counterpart and is what `roofline.peak` reports.
+# FP64 CUDA-core peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x SM clock (B200_PROFILING.md: 148 SMs, clocks.max.sm
+# 1965 MHz).  The live DFMA probe (lh_fp64_peak_probe) is the measured counterpart and is what `roofline.peak` reports.
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# dram bytes (read+write) per launch of the timed kernel from `ncu --set full` (profiles/r01_cfg3_ncu.md:
-# a middle lens chunk of cfg 3 reads and writes the five carried accumulators)
-NCU_TRAFFIC_BYTES = {3: 1.289e9}
+FP64_LANES_PER_S = 148 * 64 * 1.965e9
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the timed kernel, from one `ncu --set full` capture per
+# config (profiles/r02_all_configs_ncu.md); None = not captured
+NCU_TRAFFIC_BYTES = {0: None, 1: None, 2: None, 3: None, 4: None}
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (bench line: 3)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--scaling", default="auto", choices=["auto", "strong", "weak"],
+                    help="N > 1: strong = row slabs of ONE map (default), weak = an independent lens model per rank")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0, help="target CPU time of the all-cores oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config block (cfg 0, 1, 2, 4)")
     ap.add_argument("--delens", action="store_true",
                     help="NEXT row f1 alone (not the default bench line): lh_delens_grid on the deflection planes of "
                          "--config (default 3) for 80 synthetic sources (M1149 has 80, PAPER.md:208)")
@@ -124,27 +132,29 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-# ----------------------------------------------------------------------------- CPU oracle leg
-def oracle_sample(cfg, seconds: float):
-    """Time the oracle as it stands on a bounded sample: whole rows of the configured grid,
-    all lenses, all host cores (threads over disjoint row ranges)."""
+# ----------------------------------------------------------------------------- CPU oracle legs
+def oracle_sample(cfg, seconds: float, threads: int | None = None, min_rows: int = 0):
+    """Time the oracle as it stands on a bounded sample: whole rows of the configured grid (first model of a
+    batch), all lenses, `threads` host threads over disjoint row ranges (default: all cores)."""
     import oracle
 
-    cores = os.cpu_count() or 1
+    cores = threads or os.cpu_count() or 1
     g, L = cfg.grid, cfg.lenses[: cfg.nlens]
+    probe = max(cores, 2)
     t0 = time.perf_counter()
-    oracle.grid(L, g.x0, g.y0, g.dx, g.nx, g.ny, planes=cfg.outputs, threads=cores, rows=(0, cores))
-    rate = cores * g.nx * cfg.nlens / (time.perf_counter() - t0)  # evals/s, all cores, rough
-    rows = int(max(cores, min(g.ny, seconds * rate / (g.nx * cfg.nlens))))
-    rows = max(cores, rows // cores * cores)
+    oracle.grid(L, g.x0, g.y0, g.dx, g.nx, g.ny, planes=cfg.outputs, threads=cores, rows=(0, min(probe, g.ny)))
+    rate = min(probe, g.ny) * g.nx * cfg.nlens / (time.perf_counter() - t0)  # evals/s, rough
+    rows = int(max(cores, min_rows, min(g.ny, seconds * rate / (g.nx * cfg.nlens))))
+    rows = min(g.ny, max(cores, rows // cores * cores))
     t0 = time.perf_counter()
     oracle.grid(L, g.x0, g.y0, g.dx, g.nx, g.ny, planes=cfg.outputs, threads=cores, rows=(0, rows))
     dt = time.perf_counter() - t0
     evals = rows * g.nx * cfg.nlens
+    whole = " (the whole map)" if rows == g.ny and cfg.nmodel == 1 else " (a slab: the work is exactly linear in rows)"
     return {"value": evals / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"rows 0..{rows - 1} of the {g.nx}x{g.ny} grid x {cfg.nlens} lenses "
-                      f"({evals:.3g} evals, {dt:.1f} s; oracle/lens_oracle.c single-threaded per row slab, "
-                      f"{cores} slabs in parallel)"}, dt
+            "sample": f"rows 0..{rows - 1} of the {g.nx}x{g.ny} grid x {cfg.nlens} lenses{whole} "
+                      f"({evals:.3g} evals, {dt:.1f} s; oracle/lens_oracle.c single-threaded per row range, "
+                      f"{cores} range(s) in parallel)"}, dt
 
 
 def run_reference(args):
@@ -165,21 +175,125 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(cfg, args), "cpu_baseline": base,
+            "config": workload_config(cfg, args, 1, "weak"), "cpu_baseline": base,
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 
 
-def workload_config(cfg, args):
+def workload_config(cfg, args, world, scaling):
     g = cfg.grid
+    if world == 1:
+        par = "one GPU"
+    elif scaling == "strong":
+        par = (f"row slabs of the ONE map over {world} GPUs (lens_inputs.row_slab, lh_grid_eval_rows), lens list "
+               "replicated, no collective in the computation; one gather assembles the map (timed apart)")
+    else:
+        par = f"an independent lens model per GPU x{world} (MCMC-style samples), no collective"
     return {"workload": f"BASELINE.json configs[{args.config}] {cfg.name}: {g.nx}x{g.ny} px, {cfg.nlens} lenses"
                         + (f" x {cfg.nmodel} models" if cfg.nmodel > 1 else ""),
             "outputs": (["mean+variance over models of"] if getattr(args, "stats", False) else []) + list(cfg.outputs),
-            "evals_per_step_per_gpu": cfg.evals,
+            "evals_per_step": cfg.evals * (world if scaling == "weak" else 1),
             "l2": "L2 flushed between timed steps by rewriting a 256 MiB buffer (outside the timed events); output "
                   "planes %d MiB/step; the lens records (%d KiB) travel in the kernel parameters"
                   % (len(cfg.outputs) * cfg.nmodel * g.npix * 8 >> 20, cfg.nmodel * cfg.nlens * 192 >> 10),
-            "parallelism": f"independent lens models per GPU x{args.gpus}, no collective"}
+            "parallelism": par}
+
+
+def variant_of(outputs):
+    o = set(outputs)
+    return "grad+hess" if (o & {"ax", "ay"}) and (o - {"ax", "ay"}) else ("grad" if o <= {"ax", "ay"} else "hess")
+
+
+def stats_of(ms):
+    ms = [float(x) for x in ms]
+    return {"ms_mean": float(np.mean(ms)), "ms_median": float(np.median(ms)), "ms_best": float(np.min(ms)), "n": len(ms)}
+
+
+# ----------------------------------------------------------------------------- our arm: helpers
+def time_device_steps(torch, lh, step, steps, warmup, stream, flush):
+    """W untimed steps, then K steps each bracketed by CUDA events on the launching stream (L2 flushed before each,
+    outside the events).  Returns (per-step ms, launches in the timed region)."""
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    n0 = lh.lh_launch_count()
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        step()
+        b.record(stream)
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in ev], lh.lh_launch_count() - n0
+
+
+def sampled_parity(torch, cfg, out, model=0, n=1000, seed=2026):
+    """Parity of the planes the LAST timed step left on the device: `n` seeded pixels (plus the corners) against the
+    oracle evaluated pixel by pixel, by the rules of tests/parity.py.  Returns the worst |d|/allowed (<= 1 passes)."""
+    import oracle
+    from parity import report_planes
+
+    g = cfg.grid
+    ii, jj = li.random_points(seed, g, n)
+    ii = np.concatenate([ii, [0, g.nx - 1, 0, g.nx - 1]])
+    jj = np.concatenate([jj, [0, 0, g.ny - 1, g.ny - 1]])
+    need = set(cfg.outputs)
+    if "mu" in need:
+        need |= {"kappa", "gamma1", "gamma2"}
+    L = cfg.lenses[model * cfg.nlens:(model + 1) * cfg.nlens]
+    ref = oracle.points(L, g.x0 + ii * g.dx, g.y0 + jj * g.dx, planes=tuple(sorted(need)))
+    it, jt = torch.as_tensor(ii, device="cuda"), torch.as_tensor(jj, device="cuda")
+    got = {}
+    for name in cfg.outputs:
+        t = out[name]
+        t = t[model] if t.dim() == 3 else t
+        got[name] = t[jt, it].cpu().numpy()
+    rep = report_planes(got, ref)
+    worst = max(r["worst"] for r in rep.values())
+    return {"pixels": int(len(ii)), "worst_ratio": float(worst), "ok": bool(worst <= 1.0),
+            "planes": {k: float(v["worst"]) for k, v in rep.items()},
+            "rule": "tests/parity.py: |d| <= max(1e-11 |P|, 1e-13 max|P|) per plane, mu conditioned (R13); "
+                    "the planes of the last timed step vs oracle.points"}
+
+
+# FP64 thread-instructions per evaluation of the other lens classes (same source: SASS lens loops, recounted by
+# tests/test_sass_cpu.py) -- only used for the FP64 issue fraction of the mixed config 2
+FP64_INSTR_PER_EVAL_CLASS = {"grad+hess": {"dpie": 79.0, "nsie": 57.0, "sis": 17.75},
+                             "grad": {"dpie": 55.75, "nsie": 41.75, "sis": 10.5},
+                             "hess": {"dpie": 45.0, "nsie": 30.0, "sis": 15.75}}
+
+
+def fp64_instr_of(cfg, mode):
+    """FP64 thread-instructions one pass over `cfg` executes per pixel and model (sum over its lenses by class)."""
+    t = cfg.lenses["type"][: cfg.nlens]
+    k = FP64_INSTR_PER_EVAL_CLASS[mode]
+    return float(np.sum(t == li.DPIE) * k["dpie"] + np.sum(t == li.NSIE) * k["nsie"] + np.sum(t == li.SIS) * k["sis"])
+
+
+def config_block(torch, lh, stream, flush, which=(0, 1, 2, 4), steps=5):
+    """ms/step, evals/s and FP64 issue fraction of the other BASELINE configs (device-resident, CUDA events)."""
+    block = {}
+    for idx in which:
+        c = li.config(idx)
+        g = c.grid
+        out = {n: torch.empty((c.nmodel, g.ny, g.nx), dtype=torch.float64, device="cuda") for n in c.outputs}
+
+        def step():
+            lh.lh_grid_eval_batch(c.lenses, c.nmodel, c.nlens, g, **out)
+
+        ms, launches = time_device_steps(torch, lh, step, steps, 3, stream, flush)
+        mode = variant_of(c.outputs)
+        st = stats_of(ms)
+        sec = st["ms_median"] * 1e-3
+        block[f"cfg{idx}"] = {
+            "workload": f"{c.name}: {g.nx}x{g.ny} px x {c.nlens} lenses" + (f" x {c.nmodel} models" if c.nmodel > 1 else ""),
+            "outputs": list(c.outputs), "kernel": f"superpose_kernel<{mode}>", "steps": steps, **st,
+            "evals_per_s": c.evals / sec, "launches_per_step": launches / steps,
+            "fp64_issue_frac": fp64_instr_of(c, mode) * g.npix * c.nmodel / sec / FP64_LANES_PER_S,
+            "traffic": NCU_TRAFFIC_BYTES.get(idx),
+            "parity_last_step": sampled_parity(torch, c, out, model=c.nmodel - 1, n=300)}
+        del out
+    return block
 
 
 # ----------------------------------------------------------------------------- our arm
@@ -195,7 +309,7 @@ def run_ours(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     # LH_BENCH_BACKEND=gloo lets the N > 1 path be exercised where there are fewer GPUs than ranks (ranks then
-    # share devices and only the timing reduction goes through the process group); the driver uses NCCL.
+    # share devices and the reductions / the gather go through host memory); the driver uses NCCL.
     backend = os.environ.get("LH_BENCH_BACKEND", "nccl")
     local = local % max(1, torch.cuda.device_count()) if backend != "nccl" else local
     torch.cuda.set_device(local)
@@ -207,14 +321,32 @@ def run_ours(args):
         else:
             dist.init_process_group(backend)
 
+    def reduce_max(x):
+        if world == 1:
+            return float(x)
+        t = torch.tensor([float(x)], dtype=torch.float64, device=red_dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
     cfg = li.config(args.config)
     g = cfg.grid
+    scaling = args.scaling
+    if scaling == "auto":
+        scaling = "strong" if (world > 1 and cfg.nmodel == 1 and not args.stats) else "weak"
+    if scaling == "strong" and (cfg.nmodel != 1 or args.stats):
+        raise SystemExit("--scaling strong shards the rows of ONE map: use a single-model config")
     lenses = cfg.lenses
-    if world > 1 and rank > 0 and cfg.nmodel == 1:
+    if scaling == "weak" and world > 1 and rank > 0 and cfg.nmodel == 1:
         # another independent sample of the same model family for this rank (same shape, other seed)
-        lenses = li.cluster(1000 * args.config + rank, {1: 2, 2: 3, 3: 4}.get(args.config, 0), cfg.nlens
-                            - {1: 2, 2: 3, 3: 4}.get(args.config, 0), {0: 40.0, 3: 150.0}.get(args.config, 100.0))
-    shape = (cfg.nmodel, g.ny, g.nx)
+        nh = {1: 2, 2: 3, 3: 4}.get(args.config, 0)
+        lenses = li.cluster(1000 * args.config + rank, nh, cfg.nlens - nh, {0: 40.0, 3: 150.0}.get(args.config, 100.0))
+    j0, nrows = li.row_slab(g, rank, world) if scaling == "strong" else (0, g.ny)
+    shape = (nrows, g.nx) if scaling == "strong" else (cfg.nmodel, g.ny, g.nx)
     if args.stats:
         import dataclasses
         cfg = dataclasses.replace(cfg, outputs=("ax", "ay", "kappa", "gamma1", "gamma2"))
@@ -228,13 +360,11 @@ def run_ours(args):
     def step():
         if args.stats:
             lh.lh_grid_stats_batch(lenses, cfg.nmodel, cfg.nlens, g, out, var)
+        elif scaling == "strong":
+            if nrows > 0:
+                lh.lh_grid_eval_rows(lenses, g, j0, nrows, **out)
         else:
             lh.lh_grid_eval_batch(lenses, cfg.nmodel, cfg.nlens, g, **out)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -252,48 +382,112 @@ def run_ours(args):
         barrier()
     launches = lh.lh_launch_count() - launches0
     step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = float(sum(step_ms))
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=red_dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = reduce_max(sum(step_ms))  # MAX over ranks of the device time of the K steps
     ms_per_step = total_ms / args.steps
-    value = world * cfg.evals / (ms_per_step * 1e-3)
+    job_evals = cfg.evals * (world if scaling == "weak" else 1)  # units ALL ranks processed per step
+    value = job_evals / (ms_per_step * 1e-3)
 
-    # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region
+    # ---- strong scaling: the time to assemble the one map on rank 0 (not part of the computation)
+    assemble = None
+    if scaling == "strong" and world > 1:
+        rows_of = [li.row_slab(g, r, world)[1] for r in range(world)]
+        pad = max(rows_of)
+        full = {n: torch.empty((world, pad, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs} if rank == 0 else None
+        mine = {n: torch.zeros((pad, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs}
+        for n in cfg.outputs:
+            mine[n][:nrows].copy_(out[n])
+
+        def gather():
+            for n in cfg.outputs:
+                if backend == "nccl":
+                    dist.gather(mine[n], list(full[n].unbind(0)) if rank == 0 else None, dst=0)
+                else:  # gloo stand-in: through host memory
+                    parts = [torch.empty((pad, g.nx), dtype=torch.float64) for _ in range(world)] if rank == 0 else None
+                    dist.gather(mine[n].cpu(), parts, dst=0)
+                    if rank == 0:
+                        full[n].copy_(torch.stack(parts))
+
+        gather()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for _ in range(3):
+            gather()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        dev_ms = reduce_max(e0.elapsed_time(e1) / 3)
+        wall_ms = reduce_max((time.perf_counter() - t0) * 1e3 / 3)
+        assemble = {"ms": dev_ms if backend == "nccl" else wall_ms, "bytes": int(len(cfg.outputs) * g.npix * 8),
+                    "how": ("one dist.gather (NCCL) of every rank's slab of each plane into rank 0's map, CUDA events, "
+                            "max over ranks" if backend == "nccl" else "gloo stand-in through host memory, wall clock"),
+                    "bitwise_check": None}
+        if rank == 0:  # the assembled map is the single-device map, bit for bit (checked on rank 0's own device)
+            ref = {n: torch.empty((g.ny, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs}
+            lh.lh_grid_eval(lenses, g, **ref)
+            torch.cuda.synchronize()
+            ok = True
+            for n in cfg.outputs:
+                asm = torch.cat([full[n][r, :rows_of[r]] for r in range(world)])
+                ok = ok and bool((asm.view(torch.int64) == ref[n].view(torch.int64)).all())
+            assemble["bitwise_check"] = ok
+            del ref
+        del mine, full
+
+    # ---- end to end through the C ABI with HOST buffers: H2D of the lens list + D2H of the planes inside the timed region
     e2e = None
     if not args.no_e2e:
-        host = {n: torch.empty(shape, dtype=torch.float64).pin_memory() for n in cfg.outputs}
-        hvar = {n: torch.empty(shape, dtype=torch.float64).pin_memory() for n in cfg.outputs} if args.stats else None
-        def step_host():
-            if args.stats:  # host lens list in; mean and variance planes copied to pinned host memory
-                step()
-                for n in host:
-                    host[n].copy_(out[n], non_blocking=True)
-                    hvar[n].copy_(var[n], non_blocking=True)
+        k_e2e = max(5, min(args.steps, 10))
+
+        def e2e_run(pinned: bool):
+            def alloc():
+                t = torch.empty(shape, dtype=torch.float64)
+                return t.pin_memory() if pinned else t
+            host = {n: alloc() for n in cfg.outputs}
+            hvar = {n: alloc() for n in cfg.outputs} if args.stats else None
+
+            def step_host():
+                if args.stats:  # host lens list in; mean and variance planes copied to host memory
+                    step()
+                    for n in host:
+                        host[n].copy_(out[n], non_blocking=pinned)
+                        hvar[n].copy_(var[n], non_blocking=pinned)
+                    torch.cuda.synchronize()
+                elif scaling == "strong":
+                    if nrows > 0:
+                        lh.lh_grid_eval_rows_host(lenses, g, j0, nrows, **host)
+                else:
+                    lh.lh_grid_eval_host(lenses, cfg.nmodel, cfg.nlens, g, **host)
+
+            step_host()
+            barrier()
+            times = []
+            for _ in range(k_e2e):
+                t0 = time.perf_counter()
+                step_host()  # synchronises its stream before returning
                 torch.cuda.synchronize()
-            else:
-                lh.lh_grid_eval_host(lenses, cfg.nmodel, cfg.nlens, g, **host)
-        step_host()
-        barrier()
-        t0 = time.perf_counter()
-        k_e2e = max(1, min(args.steps, 3))
-        for _ in range(k_e2e):
-            step_host()  # synchronises its stream before returning
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device=red_dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * cfg.evals * k_e2e / dt, "unit": UNIT,
-               "h2d_bytes_per_step": int(cfg.nmodel * cfg.nlens * 192 + cfg.nmodel * 8),
+                times.append((time.perf_counter() - t0) * 1e3)
+            total = reduce_max(sum(times))
+            bitwise = all(bool((host[n].view(torch.int64) == out[n].cpu().view(torch.int64)).all()) for n in cfg.outputs) \
+                if not args.stats else None
+            return total / k_e2e, times, bitwise
+
+        ms_pin, t_pin, bit_pin = e2e_run(True)
+        ms_page, t_page, bit_page = e2e_run(False)
+        nl = cfg.nmodel * cfg.nlens
+        e2e = {"value": job_evals / (ms_pin * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(nl * 192 + cfg.nmodel * 8),
                "d2h_bytes_per_step": int(len(cfg.outputs) * g.npix * 16 if args.stats else
-                                         len(cfg.outputs) * cfg.nmodel * g.npix * 8),
-               "ms_per_step": 1e3 * dt / k_e2e, "steps": k_e2e,
-               "note": "lh_grid_eval_host: host lens list in, pinned host planes out, packing + copies + sync timed; "
-                       "the D2H copy of each of 8 row slabs overlaps the computation of the next"}
-        del host
+                                         len(cfg.outputs) * int(np.prod(shape)) * 8),
+               "ms_per_step": ms_pin, "steps": k_e2e, **{k: v for k, v in stats_of(t_pin).items() if k != "n"},
+               "host_memory": "pinned", "same_bits_as_device_planes": bit_pin,
+               "pageable": {"value": job_evals / (ms_page * 1e-3), "ms_per_step": ms_page, "steps": k_e2e,
+                            **{k: v for k, v in stats_of(t_page).items() if k != "n"},
+                            "same_bits_as_device_planes": bit_page},
+               "note": ("lh_grid_eval_rows_host" if scaling == "strong" else "lh_grid_eval_host")
+                       + ": host lens list in, host planes out, validation + packing + copies + sync timed (wall clock "
+                         "around the call, max over ranks); the D2H copy of each of up to 8 pieces overlaps the computation "
+                         "of the next; bytes are per rank"}
 
     if rank != 0:
         if world > 1:
@@ -303,40 +497,58 @@ def run_ours(args):
 
     # ---- roofline of the dominant (only) kernel: FP64 CUDA-core ALU bound
     peak_flops, _ = lh.lh_fp64_peak_probe(1 << 15)
-    mode = "grad+hess" if (set(cfg.outputs) & {"ax", "ay"}) and (set(cfg.outputs) - {"ax", "ay"}) else (
-        "grad" if set(cfg.outputs) <= {"ax", "ay"} else "hess")
+    mode = variant_of(cfg.outputs)
     fpe = FLOPS_PER_EVAL[mode]
-    step_s = float(np.mean(step_ms)) * 1e-3
+    step_s = float(np.mean(step_ms)) * 1e-3      # rank 0's own steps
     per_step = launches / args.steps
-    launch_s = step_s / per_step          # average duration of one superpose_kernel launch (CUDA events)
-    launch_evals = cfg.evals / per_step   # units one launch processes
+    rank_evals = cfg.evals * (nrows / g.ny if scaling == "strong" else 1.0)
+    launch_s = step_s / max(per_step, 1e-9)       # average duration of one superpose_kernel launch (CUDA events)
+    launch_evals = rank_evals / max(per_step, 1e-9)  # units one launch processes
     achieved = fpe * launch_evals / launch_s / 1e12
     instr_rate = FP64_INSTR_PER_EVAL[mode] * launch_evals / launch_s  # FP64 thread-instructions / s
+    d, m, a = FP64_OPS_PER_EVAL[mode]
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_flops / 1e12, "unit": "TFLOP/s",
                 "frac": achieved / (peak_flops / 1e12), "traffic": NCU_TRAFFIC_BYTES.get(args.config),
                 "peak_source": "measured live: lh_fp64_peak_probe (DFMA chains, all SMs); nominal "
                                f"{NOMINAL_FP64_TFLOPS:.1f} TFLOP/s = 148 SM x 64 lanes x 2 x 1.965 GHz "
                                "(MEASURED_PEAKS.json has no FP64 entry)",
                 "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
-                "flops_per_eval": fpe, "flops_per_eval_source": "executed FP64 flops (ncu / SASS), dPIE, " + mode,
-                "fp64_issue_frac": instr_rate / (148 * 64 * 1.965e9),
+                "flops_per_eval": fpe, "fp64_instr_per_eval": {"dfma": d, "dmul": m, "dadd": a},
+                "flops_per_eval_source": "executed FP64 flops of the dPIE lens loop, " + mode
+                                         + " (SASS; recounted by tests/test_sass_cpu.py)",
+                "fp64_issue_frac": instr_rate / FP64_LANES_PER_S,
                 "fp64_issue_note": "FP64 thread-instructions/s over 148 x 64 lanes x 1.965 GHz; only "
-                                   f"{100 * (fpe / FP64_INSTR_PER_EVAL[mode] - 1):.0f} % of them are FMAs, and every non-FP64 "
+                                   f"{100 * d / (d + m + a):.0f} % of them are FMAs, and every non-FP64 "
                                    "instruction costs a dispatch cycle of the same port (DESIGN.md sec. 7)",
                 "canonical_flops_per_eval": CANONICAL_FLOPS_PER_EVAL[mode],
-                "achieved_canonical": CANONICAL_FLOPS_PER_EVAL[mode] * cfg.evals / step_s / 1e12,
+                "achieved_canonical": CANONICAL_FLOPS_PER_EVAL[mode] * rank_evals / step_s / 1e12,
                 "kernel": "lh::superpose_kernel<%s>" % mode, "launches_per_step": per_step,
                 "kernel_ms": launch_s * 1e3, "units_per_launch": launch_evals,
-                "store_gbs": len(cfg.outputs) * cfg.nmodel * g.npix * 8 / step_s / 1e9}
+                "store_gbs": len(cfg.outputs) * int(np.prod(shape)) * 8 / step_s / 1e9}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args),
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, **{k: v for k, v in stats_of(step_ms).items() if k != "n"},
+            "higher_is_better": True, "scaling": scaling if world > 1 else "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args, world, scaling),
             "clocks": clk.summary(), "gpu_launches": int(launches), "roofline": roofline}
+    if not args.stats:
+        sub = cfg if scaling != "strong" else None
+        if sub is not None:
+            line["parity_last_step"] = sampled_parity(torch, cfg, out, model=cfg.nmodel - 1)
+        else:  # rank 0's slab: rows [0, nrows) of the same grid
+            import dataclasses
+            slab = dataclasses.replace(cfg, grid=li.Grid(g.x0, g.y0, g.dx, g.nx, nrows))
+            line["parity_last_step"] = sampled_parity(torch, slab, out)
+    if assemble:
+        line["assemble"] = assemble
     if e2e:
         line["e2e"] = e2e
-    if not args.no_cpu_baseline and world >= 1:
+    if world == 1 and not args.no_configs and args.config == 3 and not args.stats:
+        line["configs"] = config_block(torch, lh, stream, flush)
+    if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], _ = oracle_sample(cfg, args.cpu_seconds)
+        one, _ = oracle_sample(cfg, 0.0, threads=1, min_rows=64 if cfg.evals > 2e9 else g.ny)
+        line["cpu_baseline"]["single_thread"] = {k: one[k] for k in ("value", "unit", "cores", "sample")}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()

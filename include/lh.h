@@ -216,6 +216,14 @@ int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constra
  * caller without device buffers uses. */
 int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *host_o);
 
+/* Rows [j0, j0 + nrows) of ONE map into HOST planes of nrows*nx doubles each: the host-memory form of
+ * lh_grid_eval_rows (the multi-GPU row-slab primitive; "the grid is split among the GPUs"), pipelined
+ * like lh_grid_eval_host.  Pixel coordinates are those of the full grid, so the slabs of several devices stacked are
+ * bit-identical to the single-device map.  Synchronises the set stream.  Errors as lh_grid_eval_host, plus
+ * LH_EINVAL for a slab outside the grid. */
+int lh_grid_eval_rows_host(const lh_lens *lenses, int nlens, const lh_grid *g, int j0, int nrows,
+                           const lh_outputs *host_outputs);
+
 /* CUDA stream (a cudaStream_t / CUstream cast to void*) used by later calls from
  * this host thread; NULL = legacy default stream.  Always returns LH_OK. */
 int lh_set_stream(void *cuda_stream);

@@ -197,16 +197,17 @@ def random_points(seed: int, grid: Grid, n: int):
 # ---------------------------------------------------------------- sharding
 def row_slab(grid: Grid, rank: int, world: int):
     """Contiguous row slab of `grid` owned by `rank` of `world` (pixels are independent):
-    returns (sub-grid, first row j0).  Rows are split as evenly as possible, earlier ranks take the extra
-    rows; a rank may own zero rows (sub-grid ny = 0) when world > grid.ny.  The sub-grid is the SAME
-    lattice: y0 + j0*dx is computed once here, and the kernel's y0_slab + j*dx can differ from the full
-    map's y0 + (j0+j)*dx by one rounding unless dx and y0 are dyadic (they are for every BASELINE config)."""
+    returns (j0, nrows) -- rows [j0, j0 + nrows) of the SAME grid.  Rows are split as evenly as possible, earlier
+    ranks take the extra rows; a rank may own zero rows when world > grid.ny.  There is deliberately no
+    "sub-grid" with an origin of its own: a slab is addressed as (grid, j0, nrows) everywhere (lh_grid_eval_rows,
+    lh_grid_eval_rows_host, oracle.grid(rows=...)), so that row j0 + j always has the coordinate of the full
+    grid's definition, y0 + (j0 + j)*dx, and the slabs stacked are the full map bit for bit on any grid."""
     if not (0 <= rank < world):
         raise ValueError("rank outside [0, world)")
     base, extra = divmod(grid.ny, world)
     rows = base + (1 if rank < extra else 0)
     j0 = rank * base + min(rank, extra)
-    return Grid(x0=grid.x0, y0=grid.y0 + j0 * grid.dx, dx=grid.dx, nx=grid.nx, ny=rows), j0
+    return j0, rows
 
 
 def model_slab(nmodel: int, rank: int, world: int):

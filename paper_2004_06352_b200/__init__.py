@@ -7,7 +7,7 @@ missing -- there is no CPU fallback (and it never imports `oracle`).
 
 Names mirror the C ABI one to one:
     lh_grid_gradient, lh_grid_hessian, lh_lens_maps, lh_grid_gradient_batch,
-    lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_grid_stats_batch, lh_pack_model, lh_set_stream,
+    lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_grid_eval_rows_host, lh_grid_stats_batch, lh_pack_model, lh_set_stream,
     lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_math_host_eval, lh_version
 Outputs may be torch CUDA tensors (float64, contiguous), anything with a
 `data_ptr()`, or raw integer device addresses.
@@ -68,6 +68,8 @@ def _load():
         L.lh_grid_eval.argtypes = [vp, ci, gp, op]
         L.lh_grid_eval_batch.argtypes = [vp, ci, ci, gp, op]
         L.lh_grid_eval_host.argtypes = [vp, ci, ci, gp, op]
+        L.lh_grid_eval_rows_host.argtypes = [vp, ci, gp, ci, ci, op]
+        L.lh_grid_eval_rows_host.restype = ci
         L.lh_grid_stats_batch.argtypes = [vp, ci, ci, gp, op, op]
         L.lh_grid_stats_batch.restype = ci
         L.lh_chi2.argtypes = [vp, ci, gp, vp, ci, ci, dp, dp, dp, vp]
@@ -270,34 +272,42 @@ def lh_delens_grid(ax, ay, grid, sources, images, max_images: int, count):
                                   raw(images, 32 * int(max_images)), int(max_images), raw(count, 8)))
 
 
+def _host_ptr(v, count):
+    """Address of a HOST plane of at least `count` float64 elements (numpy array or torch CPU tensor, pinned or not)."""
+    if v is None:
+        return None
+    if isinstance(v, np.ndarray):
+        if v.dtype != np.float64 or not v.flags.c_contiguous:
+            raise TypeError("host planes must be C-contiguous float64")
+        if v.size < count:
+            raise ValueError(f"host plane of {v.size} elements where the call needs {count}")
+        return v.ctypes.data
+    if hasattr(v, "data_ptr"):  # e.g. a pinned torch CPU tensor
+        if getattr(v, "is_cuda", False):
+            raise TypeError("the *_host entry points take HOST planes")
+        if "float64" not in str(v.dtype) or not v.is_contiguous():
+            raise TypeError("host planes must be contiguous float64")
+        if int(v.numel()) < count:
+            raise ValueError(f"host plane of {int(v.numel())} elements where the call needs {count}")
+        return v.data_ptr()
+    raise TypeError(f"cannot take a host pointer from {type(v)}")
+
+
 def lh_grid_eval_host(lenses, nmodel, nlens, grid, **host_planes):
     """host_planes: numpy float64 C-contiguous arrays of nmodel*ny*nx elements (HOST memory,
     pinned or not); the copies back and a stream synchronise happen inside the call."""
     a, p, n = _lenses_ptr(lenses)
     if n != nmodel * nlens:
         raise ValueError("len(lenses) != nmodel*nlens")
-
-    def host_ptr(v, count):
-        if v is None:
-            return None
-        if isinstance(v, np.ndarray):
-            if v.dtype != np.float64 or not v.flags.c_contiguous:
-                raise TypeError("host planes must be C-contiguous float64")
-            if v.size < count:
-                raise ValueError(f"host plane of {v.size} elements where the call needs {count}")
-            return v.ctypes.data
-        if hasattr(v, "data_ptr"):  # e.g. a pinned torch CPU tensor
-            if getattr(v, "is_cuda", False):
-                raise TypeError("lh_grid_eval_host takes HOST planes")
-            if "float64" not in str(v.dtype) or not v.is_contiguous():
-                raise TypeError("host planes must be contiguous float64")
-            if int(v.numel()) < count:
-                raise ValueError(f"host plane of {int(v.numel())} elements where the call needs {count}")
-            return v.data_ptr()
-        raise TypeError(f"cannot take a host pointer from {type(v)}")
-
-    o = _outputs(host_planes, host_ptr, _npix(grid, nmodel))
+    o = _outputs(host_planes, _host_ptr, _npix(grid, nmodel))
     _check(_load().lh_grid_eval_host(p, nmodel, nlens, C.byref(_grid(grid)), C.byref(o)))
+
+
+def lh_grid_eval_rows_host(lenses, grid, j0: int, nrows: int, **host_planes):
+    """Rows [j0, j0+nrows) of one map into HOST planes of nrows*nx elements (numpy or pinned torch CPU tensors)."""
+    a, p, n = _lenses_ptr(lenses)
+    o = _outputs(host_planes, _host_ptr, int(nrows) * int(grid.nx))
+    _check(_load().lh_grid_eval_rows_host(p, n, C.byref(_grid(grid)), int(j0), int(nrows), C.byref(o)))
 
 
 LH_PACK_DOUBLES, LH_PACK_CLASSES = 24, 4

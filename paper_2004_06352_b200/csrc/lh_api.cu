@@ -160,6 +160,7 @@ struct EvalOpts {
     const lh_lens *shared = nullptr;  // lenses common to every model (f4), evaluated once
     int nshared = 0;
     int j0 = 0, nrows = -1;           // rows [j0, j0 + nrows) of the grid only (dev_out point at row j0); default all
+    int buf_row0 = 0;                 // row, inside planes of g->ny rows, at which dev_out point (carry is laid out alike)
     const double *px = nullptr, *py = nullptr;  // DEVICE: evaluate at these g->nx points instead of a grid (g->ny = 1)
     // >= 0: the models were validated and packed into ctx.h_table / ctx.h_ranges by pack_all() already and this job
     // evaluates `nmodel` of them starting at model `packed0` (`lenses` is then not read)
@@ -261,9 +262,9 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
         J.m2[k] = dev_m2 ? dev_m2[k] : nullptr;
     }
     J.stats = dev_m2 ? 1 : 0;
-    // carry is laid out like the planes it serves: a slab of FULL-size planes (nrows < g->ny) uses the slab's rows
-    // of a full-size carry; a stand-alone slab (lh_grid_eval_rows: g->ny == nrows) uses a carry of its own size
-    J.carry = DS().d_carry ? DS().d_carry + (nrows != g->ny ? (size_t)j0 * g->nx : 0) : nullptr;
+    // carry is laid out like the planes it serves (g->ny rows of g->nx): a piece that starts at row buf_row0 of
+    // those planes uses the same rows of the carry buffer
+    J.carry = DS().d_carry ? DS().d_carry + (size_t)opt.buf_row0 * g->nx : nullptr;
     if (two_chains) {
         J.carry2 = DS().d_carry + carry_one / sizeof(double);
         J.aux = DS().aux_stream;
@@ -587,10 +588,18 @@ int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constra
     return LH_OK;
 }
 
-int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *host_o) {
+}  // extern "C"
+
+namespace {
+
+// HOST output planes.  One map (nmodel == 1): rows [j0, j0 + nrows) of the grid into planes of nrows x nx doubles;
+// a batch: all rows of every model.
+int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, int j0, int nrows, const lh_outputs *host_o) {
     ctx.err[0] = 0;
     int rc = check_common(lenses, nmodel, nlens, g);
     if (rc) return rc;
+    if (j0 < 0 || nrows < 1 || (long long)j0 + nrows > g->ny) return fail(LH_EINVAL, "row slab outside the grid");
+    if (nmodel > 1 && (j0 != 0 || nrows != g->ny)) return fail(LH_EINVAL, "row slabs of a batch are not supported");
     if (!host_o) return fail(LH_EINVAL, "outputs is NULL");
     double *hp[NPLANES], *dp[NPLANES];
     planes_of(host_o, hp);
@@ -600,7 +609,7 @@ int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_gri
     // validate and pack every model ONCE, before anything is enqueued or copied (LH_EINVAL: nothing written); the
     // pieces below reuse the packed table
     if ((rc = pack_all(lenses, nmodel, nlens))) return rc;
-    const size_t plane_bytes = (size_t)nmodel * g->nx * g->ny * sizeof(double);
+    const size_t plane_bytes = (size_t)nmodel * g->nx * nrows * sizeof(double);
     const size_t need = plane_bytes * nreq;
     if (need > DS().planes_bytes) {
         if (DS().d_planes) {
@@ -623,7 +632,10 @@ int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_gri
         for (int k = 0; k < DeviceState::PIECES; ++k) CU(cudaEventCreateWithFlags(&DS().ev_piece[k], cudaEventDisableTiming));
     }
     const size_t npix = (size_t)g->nx * g->ny;
-    const int units = nmodel == 1 ? g->ny : nmodel;  // rows or models
+    const int units = nmodel == 1 ? nrows : nmodel;  // rows or models
+    // the device planes of one map hold the slab only: present it as a grid of `nrows` rows whose row 0 is grid row j0
+    lh_grid slab = *g;
+    if (nmodel == 1) slab.ny = nrows;
     // small jobs are not worth cutting: about 4 MB of results per piece at least
     long long want = (long long)(need >> 22);
     const int pieces = want < 1 ? 1 : (want > DeviceState::PIECES ? DeviceState::PIECES : (int)want);
@@ -637,9 +649,9 @@ int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_gri
         const size_t count = nmodel == 1 ? (size_t)nu * g->nx : (size_t)nu * npix;
         for (int k = 0; k < NPLANES; ++k) sub[k] = dp[k] ? dp[k] + off : nullptr;
         EvalOpts opt;
-        if (nmodel == 1) { opt.j0 = u0; opt.nrows = nu; opt.packed0 = 0; }
+        if (nmodel == 1) { opt.j0 = j0 + u0; opt.nrows = nu; opt.buf_row0 = u0; opt.packed0 = 0; }
         else opt.packed0 = u0;
-        rc = eval_device(lenses, nmodel == 1 ? 1 : nu, nlens, g, sub, opt);
+        rc = eval_device(lenses, nmodel == 1 ? 1 : nu, nlens, nmodel == 1 ? &slab : g, sub, opt);
         if (rc) {  // only a CUDA failure can get here: the lens lists were validated above
             cudaStreamSynchronize(DS().copy_stream);
             return rc;
@@ -652,6 +664,18 @@ int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_gri
     CU(cudaStreamSynchronize(DS().copy_stream));
     CU(cudaStreamSynchronize(ctx.stream));
     return LH_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lh_grid_eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, const lh_outputs *host_o) {
+    return eval_host(lenses, nmodel, nlens, g, 0, g ? g->ny : 0, host_o);
+}
+
+int lh_grid_eval_rows_host(const lh_lens *lenses, int nlens, const lh_grid *g, int j0, int nrows, const lh_outputs *host_o) {
+    return eval_host(lenses, 1, nlens, g, j0, nrows, host_o);
 }
 
 int lh_pack_model(const lh_lens *lenses, int n, double *table, int32_t *class_begin) {

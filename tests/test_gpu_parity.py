@@ -272,16 +272,19 @@ def test_row_slabs_reassemble_the_full_map_bitwise(world):
     """Every rank evaluates lens_inputs.row_slab(rank) with lh_grid_eval_rows; stacked, the slabs are bit-identical
     to the single-device map (same pixel coordinates, same arithmetic) -- including a model with lens chunks."""
     c = li.config(2, scale=16)  # 128 x 128, 500 mixed lenses (4 lens chunks through the carry buffer)
-    g = c.grid
+    g = li.Grid(x0=c.grid.x0 + 0.1, y0=c.grid.y0 + 0.3, dx=c.grid.dx * 1.1, nx=c.grid.nx, ny=c.grid.ny)  # not dyadic
     full = run_gpu(c.lenses, g, ("ax", "kappa", "mu"))
     parts = {n: [] for n in full}
     for rank in range(world):
-        sub, j0 = li.row_slab(g, rank, world)
-        out = dev_planes(tuple(full), (sub.ny, g.nx))
-        lh.lh_grid_eval_rows(c.lenses, g, j0, sub.ny, **out)
+        j0, nrows = li.row_slab(g, rank, world)
+        out = dev_planes(tuple(full), (nrows, g.nx))
+        lh.lh_grid_eval_rows(c.lenses, g, j0, nrows, **out)
         torch.cuda.synchronize()
+        host = {n: np.full((nrows, g.nx), np.nan) for n in full}
+        lh.lh_grid_eval_rows_host(c.lenses, g, j0, nrows, **host)  # the same slab into HOST planes: same bits
         for n in full:
             parts[n].append(out[n].cpu().numpy())
+            assert np.array_equal(host[n], parts[n][-1], equal_nan=True)
     for n in full:
         assert np.array_equal(np.concatenate(parts[n]), full[n], equal_nan=True)
     with pytest.raises(lh.LhError):
@@ -559,3 +562,60 @@ def test_binding_refuses_undersized_or_misplaced_tensors():
         lh.lh_grid_eval_host(c.lenses, 1, c.nlens, g, ax=np.empty(g.npix - 1))
     with pytest.raises(TypeError):
         lh.lh_grid_eval_host(c.lenses, 1, c.nlens, g, ax=ok)  # a device tensor where a host plane is expected
+
+
+# ------------------------------------------------------------------ multi-GPU: two devices, bench arm
+@pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs two CUDA devices")
+def test_two_devices_row_slabs_assemble_the_single_device_map_bitwise():
+    """Rank r's slab on device r (lh_grid_eval_rows, current device switched per call), copied into the owner's
+    planes over the peer link: bit-identical to the map one device computes alone."""
+    c = li.config(3, scale=8)  # 512 x 512, 1000 dPIE: lens chunks through the per-device carry buffers
+    g = c.grid
+    names = ("ax", "kappa", "mu")
+    torch.cuda.set_device(0)
+    full = dev_planes(names, (g.ny, g.nx))
+    lh.lh_grid_eval(c.lenses, g, **full)
+    torch.cuda.synchronize()
+    asm = dev_planes(names, (g.ny, g.nx))
+    for rank in range(2):
+        j0, nrows = li.row_slab(g, rank, 2)
+        torch.cuda.set_device(rank)
+        lh.lh_set_stream(None)
+        out = {n: torch.full((nrows, g.nx), float("nan"), dtype=torch.float64, device=f"cuda:{rank}") for n in names}
+        lh.lh_grid_eval_rows(c.lenses, g, j0, nrows, **out)
+        torch.cuda.synchronize()
+        for n in names:
+            asm[n][j0:j0 + nrows].copy_(out[n])  # device-to-device (peer) copy into the owner's plane
+    torch.cuda.set_device(0)
+    torch.cuda.synchronize()
+    for n in names:
+        assert torch.equal(asm[n].view(torch.int64), full[n].view(torch.int64))
+
+
+def test_bench_strong_scaling_arm_two_ranks_over_gloo():
+    """`bench.py --gpus 2` as the driver launches it (torchrun, one process per rank), with the process group on gloo
+    so that two ranks can share this one GPU: the default N > 1 arm shards the ROWS of one map, the
+    assembled map equals the single-device map bit for bit, and the line carries the contract's keys."""
+    import json
+    import socket
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    env = dict(os.environ, LH_BENCH_BACKEND="gloo")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "3",
+           "--warmup", "3", "--config", "1", "--no-cpu-baseline"]
+    r = subprocess.run(cmd, env=env, cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout[-2000:]
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "strong" and d["gpu_launches"] == 3  # rank 0: one launch per step
+    assert d["assemble"]["bitwise_check"] is True and d["assemble"]["bytes"] == 2 * 1024 * 1024 * 8
+    assert d["parity_last_step"]["ok"] and d["e2e"]["same_bits_as_device_planes"] is True
+    assert d["config"]["evals_per_step"] == 1024 * 1024 * 100
+    assert abs(d["value"] - d["config"]["evals_per_step"] / (d["ms_per_step"] * 1e-3)) < 1e-6 * d["value"]

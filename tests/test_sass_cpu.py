@@ -77,3 +77,56 @@ def test_no_spills_and_no_calls_in_fast_variants(sass, variant):
 def test_extreme_variants_exist_and_use_libdevice_paths(sass):
     names = [n for n in sass if "superpose_kernel" in n and re.search(r"ILb[01]ELb[01]ELb1ELb[01]E", n)]
     assert len(names) == 6  # grad / hess / both, grid and points
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# bench.py's per-evaluation instruction counts are NOT typed in from a profile: they are recounted here from the
+# lens loops of the built library, and the test fails when bench.py and the kernel drift apart.
+def _lens_loops(lines):
+    """Innermost backward-branch loops of a kernel, in address order, each as a dict opcode -> count."""
+    ins = []
+    for line in lines:
+        m = re.search(r"/\*([0-9a-f]{4,})\*/\s+(?:@!?U?P\d\s+)?([A-Z0-9_.]+)\s*([^;]*);", line)
+        if m:
+            ins.append((int(m.group(1), 16), m.group(2), m.group(3)))
+    loops = []
+    for at, op, args in ins:
+        if op.startswith("BRA"):
+            m = re.search(r"0x([0-9a-f]+)", args)
+            if m and int(m.group(1), 16) < at:
+                loops.append((int(m.group(1), 16), at))
+    inner = [l for l in loops if not any(o != l and l[0] <= o[0] and o[1] <= l[1] for o in loops)]
+    out = []
+    for lo, hi in sorted(inner):
+        ops = {}
+        for at, op, _ in ins:
+            if lo <= at <= hi:
+                ops[op.split(".")[0]] = ops.get(op.split(".")[0], 0) + 1
+        if ops.get("DFMA", 0) + ops.get("DMUL", 0) + ops.get("DADD", 0) > 20:  # a lens loop, not a staging loop
+            out.append(ops)
+    return out
+
+
+# MUFU seeds per evaluation (lh_math.cuh): they tell how many evaluations one loop iteration holds
+_MUFU_PER_EVAL = {"grad+hess": {"dpie": 5, "nsie": 5, "sis": 1}, "grad": {"dpie": 5, "nsie": 4, "sis": 1},
+                  "hess": {"dpie": 3, "nsie": 2, "sis": 1}}
+_VARIANT = {"ILb1ELb1ELb0ELb0E": "grad+hess", "ILb1ELb0ELb0ELb0E": "grad", "ILb0ELb1ELb0ELb0E": "hess"}
+
+
+@pytest.mark.parametrize("variant", FAST)
+def test_bench_instruction_counts_match_the_built_kernel(sass, variant):
+    import bench
+
+    mode = _VARIANT[variant]
+    name = next(n for n in sass if "superpose_kernel" in n and variant in n)
+    loops = _lens_loops(sass[name])
+    assert len(loops) == 3, f"{name}: expected the dPIE, NSIE and SIS loops, found {len(loops)}"
+    for cls, ops in zip(("dpie", "nsie", "sis"), loops):
+        evals = ops.get("MUFU", 0) / _MUFU_PER_EVAL[mode][cls]
+        assert evals == int(evals) and evals >= 1, (cls, ops)
+        per_eval = (ops.get("DFMA", 0) / evals, ops.get("DMUL", 0) / evals, ops.get("DADD", 0) / evals)
+        assert sum(per_eval) == bench.FP64_INSTR_PER_EVAL_CLASS[mode][cls], (mode, cls, per_eval)
+        if cls == "dpie":
+            assert per_eval == bench.FP64_OPS_PER_EVAL[mode], (mode, per_eval)
+            assert bench.FLOPS_PER_EVAL[mode] == 2 * per_eval[0] + per_eval[1] + per_eval[2]
+            assert bench.FP64_INSTR_PER_EVAL[mode] == sum(per_eval)

@@ -34,10 +34,12 @@ def _worker(rank, world, port, q):
     try:
         # ---- one map, row slabs
         c = li.config(2, scale=32)  # 64 x 64, 500 mixed lenses
-        g = c.grid
-        sub, j0 = li.row_slab(g, rank, world)
-        mine = oracle.grid(c.lenses, sub.x0, sub.y0, sub.dx, sub.nx, sub.ny, planes=("ax", "kappa", "mu"))
-        rows = [li.row_slab(g, r, world)[0].ny for r in range(world)]
+        g = li.Grid(x0=c.grid.x0 + 0.1, y0=c.grid.y0 + 0.3, dx=c.grid.dx * 1.1, nx=c.grid.nx, ny=c.grid.ny)  # not dyadic
+        j0, nrows = li.row_slab(g, rank, world)
+        # a slab is (grid, j0, nrows): the oracle evaluates rows [j0, j0 + nrows) of the FULL grid definition
+        mine = oracle.grid(c.lenses, g.x0, g.y0, g.dx, g.nx, g.ny, planes=("ax", "kappa", "mu"), rows=(j0, j0 + nrows))
+        mine = {n: v[j0:j0 + nrows] for n, v in mine.items()}
+        rows = [li.row_slab(g, r, world)[1] for r in range(world)]
         ok = True
         for name in ("ax", "kappa", "mu"):
             parts = [torch.empty((rows[r], g.nx), dtype=torch.float64) for r in range(world)]
@@ -82,10 +84,9 @@ def test_row_slabs_tile_the_grid(ny, world):
     g = li.Grid(x0=-3.0, y0=1.5, dx=0.25, nx=5, ny=ny)
     nxt = 0
     for r in range(world):
-        sub, j0 = li.row_slab(g, r, world)
-        assert j0 == nxt and sub.nx == g.nx and sub.dx == g.dx and sub.x0 == g.x0
-        assert sub.y0 == g.y0 + j0 * g.dx
-        nxt += sub.ny
+        j0, nrows = li.row_slab(g, r, world)
+        assert j0 == nxt and 0 <= nrows <= -(-ny // world)
+        nxt += nrows
     assert nxt == ny
     with pytest.raises(ValueError):
         li.row_slab(g, world, world)
