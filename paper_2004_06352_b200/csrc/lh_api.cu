@@ -227,8 +227,10 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     const size_t carry_one =
         (nlens > lh::LAUNCH_RECORDS || nshared > 0) ? (size_t)5 * g->nx * g->ny * sizeof(double) : 0;
     // batches of chunked models run as two interleaved launch chains, each with a carry buffer of its own
-    const bool two_chains = nlens > lh::LAUNCH_RECORDS && nmodel > 1 && !dev_m2 && nshared == 0;
-    const size_t carry_need = carry_one * (two_chains ? 2 : 1);
+    // (statistics: the odd-model chain folds into scratch planes kept behind the two carry buffers)
+    const bool two_chains = nlens > lh::LAUNCH_RECORDS && nmodel > 1 && nshared == 0;
+    const size_t stats_scratch = (two_chains && dev_m2) ? (size_t)18 * g->nx * g->ny * sizeof(double) : 0;
+    const size_t carry_need = carry_one * (two_chains ? 2 : 1) + stats_scratch;
     if (two_chains && !DS().aux_stream) {
         CU(cudaStreamCreateWithFlags(&DS().aux_stream, cudaStreamNonBlocking));
         CU(cudaEventCreateWithFlags(&DS().ev_fork, cudaEventDisableTiming));
@@ -270,6 +272,7 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
         J.aux = DS().aux_stream;
         J.ev_fork = DS().ev_fork;
         J.ev_join = DS().ev_join;
+        if (stats_scratch) J.stats_scratch = DS().d_carry + 2 * (carry_one / sizeof(double));
     }
     CU(lh::launch_eval(J, s, &ctx.launches));
     if (carry_need) {

@@ -6,10 +6,10 @@
 //   "searching for the images by delensing and checking the grid for sources ... Each image found is
 //    stored ... divergent execution path"                               PAPER.md:194 (sec. 4.2)
 //
-// One thread owns one grid cell (two triangles, cut along V10-V01).  The sources of a launch
-// travel in the kernel parameters, so the source index is warp-uniform and each source reaches the
-// comparisons as a uniform operand; a cell first rejects a source against the bounding box of its
-// four source-plane corners (the common, convergent path: that box contains the boxes of both
+// One thread owns one grid cell (two triangles, cut along V10-V01); a CTA owns a tile of 32 x 8 cells.
+// The sources of a launch travel in the kernel parameters.  A tile first keeps the sources that fall in
+// the bounding box of ALL its cells' source-plane corners (shared memory list, typically empty); a cell
+// then rejects those against the box of its own four corners (that box contains the boxes of both
 // triangles, so nothing the definition accepts is lost) and only then runs, per triangle, the
 // definition of R22: closed bounding box of the three vertices AND the barycentric test.  The test arithmetic is written with the round-to-nearest intrinsics, i.e. WITHOUT FMA
 // contraction: it takes an integer decision (inside / outside) and must take it in exactly the
@@ -69,32 +69,97 @@ __device__ __forceinline__ void test_triangle(const DelensParams &P, int s, doub
     P.images[k] = im;
 }
 
+// A CTA owns a tile of TILE_CW x TILE_CH cells (one warp per cell row, coalesced vertex loads) and walks the tiles
+// of the grid persistently.  Per tile: (1) every thread maps the four corners of its cell to the source plane and
+// takes their bounding box; (2) the boxes are reduced to the box of the TILE; (3) the threads scan the source list
+// together and keep, in shared memory, the few sources inside the tile's box; (4) every thread runs the R22 test of
+// its cell against those survivors only.  Steps (2)-(3) are a superset filter (a source outside the tile's box is
+// outside the box of each of its cells), so the images found are exactly those of the plain cell x source loop.
+constexpr int TILE_CW = 32, TILE_CH = DELENS_THREADS / 32;
+
+__device__ __forceinline__ double warp_min(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
 template <bool DEV_SRC>
 __global__ void __launch_bounds__(DELENS_THREADS) delens_kernel(const __grid_constant__ DelensParams P) {
-    const long long ncx = P.nx - 1, ncells = ncx * (P.ny - 1);
-    for (long long cell = (long long)blockIdx.x * DELENS_THREADS + threadIdx.x; cell < ncells;
-         cell += (long long)gridDim.x * DELENS_THREADS) {
-        const int j = (int)(cell / ncx), i = (int)(cell - (long long)j * ncx);
+    __shared__ double s_part[TILE_CH][4];     // per-warp box: lox, hix, loy, hiy
+    __shared__ double s_box[4];               // box of the tile
+    __shared__ int s_n;                       // survivors of the current pass
+    __shared__ int s_idx[DELENS_SOURCES];     // their indices into the launch's source list
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int ncx = P.nx - 1, ncy = P.ny - 1;
+    const int tiles_x = (ncx + TILE_CW - 1) / TILE_CW, tiles_y = (ncy + TILE_CH - 1) / TILE_CH;
+    const long long ntiles = (long long)tiles_x * tiles_y;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int ty = (int)(tile / tiles_x), tx = (int)(tile - (long long)ty * tiles_x);
+        const int i = tx * TILE_CW + lane, j = ty * TILE_CH + warp;
+        const bool valid = i < ncx && j < ncy;
+        const long long cell = (long long)j * ncx + i;
         double T[4][2], B[4][2];  // corners 00, 10, 01, 11 in the image plane and in the source plane
-        double lox = 1e300, hix = -1e300, loy = 1e300, hiy = -1e300;
+        double lox = INFINITY, hix = -INFINITY, loy = INFINITY, hiy = -INFINITY;
+        if (valid) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            const int ii = i + (c & 1), jj = j + (c >> 1);
-            const size_t p = (size_t)jj * P.nx + ii;
-            T[c][0] = __dadd_rn(P.x0, __dmul_rn((double)ii, P.dx));
-            T[c][1] = __dadd_rn(P.y0, __dmul_rn((double)jj, P.dx));
-            B[c][0] = __dsub_rn(T[c][0], __ldg(P.ax + p));
-            B[c][1] = __dsub_rn(T[c][1], __ldg(P.ay + p));
-            lox = fmin(lox, B[c][0]); hix = fmax(hix, B[c][0]);
-            loy = fmin(loy, B[c][1]); hiy = fmax(hiy, B[c][1]);
+            for (int c = 0; c < 4; ++c) {
+                const int ii = i + (c & 1), jj = j + (c >> 1);
+                const size_t p = (size_t)jj * P.nx + ii;
+                T[c][0] = __dadd_rn(P.x0, __dmul_rn((double)ii, P.dx));
+                T[c][1] = __dadd_rn(P.y0, __dmul_rn((double)jj, P.dx));
+                B[c][0] = __dsub_rn(T[c][0], __ldg(P.ax + p));
+                B[c][1] = __dsub_rn(T[c][1], __ldg(P.ay + p));
+                lox = fmin(lox, B[c][0]); hix = fmax(hix, B[c][0]);
+                loy = fmin(loy, B[c][1]); hiy = fmax(hiy, B[c][1]);
+            }
         }
-        for (int s = 0; s < P.nsources; ++s) {
-            const double sx = DEV_SRC ? __ldg(P.dsrc + 2 * s) : P.src[s][0];
-            const double sy = DEV_SRC ? __ldg(P.dsrc + 2 * s + 1) : P.src[s][1];
-            // outside the box of the four corners = outside the box of either triangle (R22): reject
-            if (sx < lox || sx > hix || sy < loy || sy > hiy) continue;
-            test_triangle(P, s, sx, sy, T, B, 0, 1, 2, 2 * cell);
-            test_triangle(P, s, sx, sy, T, B, 3, 2, 1, 2 * cell + 1);
+        // (2) box of the tile.  fmin / fmax drop NaN corners (a NaN deflection never yields an image: every
+        // comparison of the cell's own test below is false for it)
+        {
+            const double a = warp_min(lox), b = warp_max(hix), c = warp_min(loy), d = warp_max(hiy);
+            if (lane == 0) { s_part[warp][0] = a; s_part[warp][1] = b; s_part[warp][2] = c; s_part[warp][3] = d; }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double a = s_part[0][0], b = s_part[0][1], c = s_part[0][2], d = s_part[0][3];
+            for (int w = 1; w < TILE_CH; ++w) {
+                a = fmin(a, s_part[w][0]); b = fmax(b, s_part[w][1]);
+                c = fmin(c, s_part[w][2]); d = fmax(d, s_part[w][3]);
+            }
+            s_box[0] = a; s_box[1] = b; s_box[2] = c; s_box[3] = d;
+        }
+        // DEV_SRC: the device list may be longer than one pass holds
+        for (int s0 = 0; s0 < P.nsources; s0 += DELENS_SOURCES) {
+            const int ns = P.nsources - s0 < DELENS_SOURCES ? P.nsources - s0 : DELENS_SOURCES;
+            if (threadIdx.x == 0) s_n = 0;
+            __syncthreads();
+            // (3) sources inside the tile's box (NaN sources -- chi^2 sources without constraints -- fail the test)
+            const double tlox = s_box[0], thix = s_box[1], tloy = s_box[2], thiy = s_box[3];
+            for (int s = threadIdx.x; s < ns; s += DELENS_THREADS) {
+                const double sx = DEV_SRC ? __ldg(P.dsrc + 2 * (s0 + s)) : P.src[s][0];
+                const double sy = DEV_SRC ? __ldg(P.dsrc + 2 * (s0 + s) + 1) : P.src[s][1];
+                if (sx >= tlox && sx <= thix && sy >= tloy && sy <= thiy) s_idx[atomicAdd(&s_n, 1)] = s;
+            }
+            __syncthreads();
+            // (4) the cell's own test on the survivors
+            const int n = s_n;
+            if (valid) {
+                for (int q = 0; q < n; ++q) {
+                    const int s = s_idx[q];
+                    const double sx = DEV_SRC ? __ldg(P.dsrc + 2 * (s0 + s)) : P.src[s][0];
+                    const double sy = DEV_SRC ? __ldg(P.dsrc + 2 * (s0 + s) + 1) : P.src[s][1];
+                    // outside the box of the four corners = outside the box of either triangle (R22): reject
+                    if (sx < lox || sx > hix || sy < loy || sy > hiy) continue;
+                    test_triangle(P, s0 + s, sx, sy, T, B, 0, 1, 2, 2 * cell);
+                    test_triangle(P, s0 + s, sx, sy, T, B, 3, 2, 1, 2 * cell + 1);
+                }
+            }
+            __syncthreads();  // s_n / s_idx / s_box are rewritten by the next pass or tile
         }
     }
 }
@@ -128,7 +193,7 @@ cudaError_t launch_delens(const double *ax, const double *ay, double x0, double 
     P.x0 = x0; P.y0 = y0; P.dx = dx; P.nx = nx; P.ny = ny;
     const long long ncells = (long long)(nx - 1) * (ny - 1);
     if (ncells <= 0) return cudaSuccess;
-    long long blocks = (ncells + DELENS_THREADS - 1) / DELENS_THREADS;
+    long long blocks = (long long)((nx - 1 + TILE_CW - 1) / TILE_CW) * ((ny - 1 + TILE_CH - 1) / TILE_CH);
     if (blocks > (long long)sms * 8) blocks = (long long)sms * 8;  // persistent: 8 CTAs of 256 threads per SM
     for (int s0 = 0; s0 < ns; s0 += DELENS_SOURCES) {
         const int n = ns - s0 < DELENS_SOURCES ? ns - s0 : DELENS_SOURCES;
@@ -153,7 +218,7 @@ cudaError_t launch_delens_dev(const double *ax, const double *ay, double x0, dou
     P.source0 = 0; P.nsources = ns; P.dsrc = dsources;
     const long long ncells = (long long)(nx - 1) * (ny - 1);
     if (ncells <= 0 || ns <= 0) return cudaSuccess;
-    long long blocks = (ncells + DELENS_THREADS - 1) / DELENS_THREADS;
+    long long blocks = (long long)((nx - 1 + TILE_CW - 1) / TILE_CW) * ((ny - 1 + TILE_CH - 1) / TILE_CH);
     if (blocks > (long long)sms * 8) blocks = (long long)sms * 8;
     delens_kernel<true><<<(unsigned)blocks, DELENS_THREADS, 0, st>>>(P);
     ++*launches;

@@ -340,8 +340,9 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
     if (P.stats) {
         // f2: running mean / variance over the models of a batch (Welford), one model per launch
         // (blockIdx.y == 0), so a pixel is updated by exactly one thread per launch and launches
-        // are ordered by the stream.  n = models seen including this one.
-        const double n = (double)(P.model0 + 1);
+        // are ordered by the stream.  n = models folded into THESE planes including this one (a batch of chunked
+        // models keeps two sets of running planes, one per launch chain; merge_stats_kernel joins them).
+        const double n = (double)P.stats_n;
 #pragma unroll
         for (int pl = 0; pl < 9; ++pl) {
             if ((pl < 2 && !GRAD) || (pl >= 2 && !HESS)) continue;
@@ -351,7 +352,7 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
             for (int k = 0; k < PX; ++k) {
                 if (i0 + k >= P.nx) continue;
                 double mean = 0.0, m2 = 0.0;
-                if (P.model0 > 0) {
+                if (P.stats_n > 1) {
                     mean = o[pix + k];
                     if (q) m2 = q[pix + k];
                 }
@@ -380,6 +381,28 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
                 if (i0 + k < P.nx) o[idx + k] = v[pl][k];
                 if (i0 + k + 1 < P.nx) o[idx + k + 1] = v[pl][k + 1];
             }
+        }
+    }
+}
+
+// f2, two launch chains: join the running statistics of the even models (n0 of them, in the caller's planes) and of
+// the odd models (n1, scratch planes) -- the pairwise update of Chan, Golub & LeVeque:
+//   d = mean1 - mean0;  mean = mean0 + d n1/n;  M2 = M2_0 + M2_1 + d^2 n0 n1/n;  variance = M2/n  (population, R21)
+struct MergeParams {
+    double *mean0[9], *m20[9];
+    const double *mean1[9], *m21[9];
+    int n0, n1;
+    long long npix;
+};
+__global__ void __launch_bounds__(256) merge_stats_kernel(const MergeParams M) {
+    const double n0 = (double)M.n0, n1 = (double)M.n1, n = n0 + n1;
+    for (long long p = (long long)blockIdx.x * 256 + threadIdx.x; p < M.npix; p += (long long)gridDim.x * 256) {
+#pragma unroll
+        for (int k = 0; k < 9; ++k) {
+            if (!M.mean0[k]) continue;
+            const double a = M.mean0[k][p], d = M.mean1[k][p] - a;
+            M.mean0[k][p] = a + d * (n1 / n);
+            if (M.m20[k]) M.m20[k][p] = (M.m20[k][p] + M.m21[k][p] + d * d * (n0 * n1 / n)) / n;
         }
     }
 }
@@ -430,6 +453,7 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     };
 
     const int n = J.nlens;
+    int stats_n_of_chunked = 0;  // != 0: the Welford count of the next chunked model (two-chain statistics)
     // lens chunks [lo, hi) of one packed model -> consecutive launches of a single model slot
     auto chunks = [&](const LensK *table, const ModelRanges &rg, int count, int model, bool first_is_first, bool last_is_last,
                       int stats) -> cudaError_t {
@@ -446,6 +470,8 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
             Q.model0 = model; Q.stride = hi - lo;
             Q.first = (c == 0) && first_is_first; Q.last = (c == nch - 1) && last_is_last;
             Q.stats = stats;
+            if (stats_n_of_chunked) Q.stats_n = stats_n_of_chunked;
+            else Q.stats_n = model + 1;
             cudaError_t e = go(1, extreme);
             if (e != cudaSuccess) return e;
         }
@@ -471,6 +497,7 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
             if (n > 0) std::memcpy(Q.table, J.table + (size_t)m0 * n, (size_t)nm * n * sizeof(LensK));
             Q.model0 = m0; Q.stride = n; Q.first = shared ? 0 : 1; Q.last = 1;
             Q.stats = J.stats ? ((m0 == J.nmodel - 1) ? 2 : 1) : 0;
+            Q.stats_n = m0 + 1;
             cudaError_t e = go(nm, extreme);
             if (e != cudaSuccess) return e;
         }
@@ -481,17 +508,30 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     // independent chains, so the partial last wave of one chain's launch is filled by the other chain's CTAs
     // (cfg 4: 4096 CTAs over 888 resident slots = 4.6 waves per launch).  Statistics mode folds the models in order
     // and stays on one stream.
-    const bool two = J.aux != nullptr && J.carry2 != nullptr && J.nmodel > 1 && !J.stats;
+    const bool two = J.aux != nullptr && J.carry2 != nullptr && J.nmodel > 1 && (!J.stats || J.stats_scratch != nullptr);
     cudaError_t e = cudaSuccess;
     if (two) {
         if ((e = cudaEventRecord(J.ev_fork, stream)) != cudaSuccess) return e;
         if ((e = cudaStreamWaitEvent(J.aux, J.ev_fork, 0)) != cudaSuccess) return e;
     }
+    // two-chain statistics: the even models fold into the caller's mean / m2 planes, the odd ones into scratch planes
+    // [k] = mean of plane k, [9 + k] = m2 of plane k; merge_stats_kernel joins the two (Chan et al. pairwise update)
+    double *out1[9], *m2_1[9];
+    for (int k = 0; k < 9; ++k) {
+        out1[k] = (J.stats && two && J.out[k]) ? J.stats_scratch + (size_t)k * J.plane : nullptr;
+        m2_1[k] = (J.stats && two && J.m2[k]) ? J.stats_scratch + (size_t)(9 + k) * J.plane : nullptr;
+    }
     for (int m = 0; m < J.nmodel && e == cudaSuccess; ++m) {
         const bool odd = two && (m & 1);
         cur = odd ? J.aux : stream;
         Q.carry = odd ? J.carry2 : J.carry;
-        e = chunks(J.table + (size_t)m * n, J.ranges[m], n, m, true, true, J.stats ? ((m == J.nmodel - 1) ? 2 : 1) : 0);
+        int st = J.stats ? ((m == J.nmodel - 1) ? 2 : 1) : 0;
+        if (J.stats && two) {
+            st = 1;  // never finalised in the kernel: the merge divides by the count
+            stats_n_of_chunked = (m >> 1) + 1;
+            for (int k = 0; k < 9; ++k) { Q.out[k] = odd ? out1[k] : J.out[k]; Q.m2[k] = odd ? m2_1[k] : J.m2[k]; }
+        }
+        e = chunks(J.table + (size_t)m * n, J.ranges[m], n, m, true, true, st);
     }
     cur = stream;
     Q.carry = J.carry;
@@ -499,6 +539,16 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
         cudaError_t e2 = cudaEventRecord(J.ev_join, J.aux);
         if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(stream, J.ev_join, 0);
         if (e == cudaSuccess) e = e2;
+    }
+    if (e == cudaSuccess && J.stats && two) {
+        MergeParams M;
+        for (int k = 0; k < 9; ++k) { M.mean0[k] = J.out[k]; M.m20[k] = J.m2[k]; M.mean1[k] = out1[k]; M.m21[k] = m2_1[k]; }
+        M.n0 = (J.nmodel + 1) / 2; M.n1 = J.nmodel / 2;
+        M.npix = (long long)J.nx * J.ny;
+        const long long blocks = (M.npix + 255) / 256;
+        merge_stats_kernel<<<(unsigned)(blocks > 65535LL * 16 ? 65535LL * 16 : blocks), 256, 0, stream>>>(M);
+        ++*launches;
+        e = cudaGetLastError();
     }
     return e;
 }

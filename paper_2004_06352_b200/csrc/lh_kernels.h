@@ -23,6 +23,7 @@ struct LaunchParams {
     int model0;              // global index of the launch's first model (blockIdx.y = model - model0)
     int stride;              // records per model in table[]
     int first, last;         // this launch holds the first / last lens chunk of its model(s)
+    int stats_n;             // stats only: models folded into out[] / m2[] including this launch's
     int stats;               // 0: out[] are per-model planes.  1 / 2: out[] are running MEANS over models and m2[] the
                              // running sums of squared deviations (Welford); 2 = last model: m2[] is divided by the count
     double *m2[9];           // stats only; nullptr = variance of that plane not wanted
@@ -57,6 +58,7 @@ struct EvalJob {
     double *carry2 = nullptr;
     cudaStream_t aux = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    double *stats_scratch = nullptr;  // stats + two chains: DEVICE, 18 planes (mean, m2 of the odd-model chain)
 };
 
 // Enqueues every launch of the job on `stream`; adds the number of kernels launched to *launches.
