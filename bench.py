@@ -79,6 +79,9 @@ def parse():
     ap.add_argument("--chi2", action="store_true",
                     help="NEXT row f3 alone (not the default bench line): lh_chi2 on --config (default 3) with 80 "
                          "sources / 227 image constraints (the shape of M1149, PAPER.md:208) at seeded random positions")
+    ap.add_argument("--shared", action="store_true",
+                    help="NEXT row f4 on config 4 (not the default bench line): the 298 galaxies the 64 models have in common "
+                         "are evaluated once (lh_grid_eval_batch_shared), each model adds its 2 halos")
     ap.add_argument("--stats", action="store_true",
                     help="NEXT row f2 on a batch config (use --config 4): per-pixel mean and variance of ax ay kappa "
                          "gamma1 gamma2 over the models through lh_grid_stats_batch (not the default bench line)")
@@ -598,6 +601,42 @@ def run_chi2(args):
     print(json.dumps(line), flush=True)
 
 
+def run_shared(args):
+    """f4 measured alone: one step = lh_grid_eval_batch_shared on config 4 (shared galaxies once + 2 halos per model),
+    reported apart from the headline as SURVEY.md sec. 8(a6) asks: it is NOT the 2.0e10-evaluation workload of cfg 4."""
+    import torch
+
+    import paper_2004_06352_b200 as lh
+
+    torch.cuda.set_device(0)
+    c = li.config(4)
+    g = c.grid
+    L = c.lenses.reshape(c.nmodel, c.nlens)
+    shared, varying = L[0, 2:].copy(), np.ascontiguousarray(L[:, :2]).reshape(-1)
+    assert all(np.array_equal(L[m, 2:], shared) for m in range(c.nmodel))
+    out = {n: torch.empty((c.nmodel, g.ny, g.nx), dtype=torch.float64, device="cuda") for n in c.outputs}
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+    lh.lh_set_stream(stream)
+
+    def step():
+        lh.lh_grid_eval_batch_shared(shared, varying, c.nmodel, 2, g, **out)
+
+    with ClockSampler(0) as clk:
+        ms, launches = time_device_steps(torch, lh, step, args.steps, max(args.warmup, 3), stream, flush)
+    st = stats_of(ms)
+    done = g.npix * (len(shared) + 2 * c.nmodel)  # evaluations actually executed
+    line = {"metric": "shared-lens batch, maps/sec (64 models of 300 lenses, 298 shared)", "value": c.nmodel / (st["ms_mean"] * 1e-3),
+            "unit": "model maps/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": st["ms_mean"],
+            **{k: v for k, v in st.items() if k != "n"}, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"NEXT row f4: configs[4] {g.nx}x{g.ny} px, {c.nmodel} models = {len(shared)} shared + 2 own lenses"},
+            "evals_executed_per_step": int(done), "evals_of_the_plain_batch": int(c.evals),
+            "executed_evals_per_s": done / (st["ms_mean"] * 1e-3), "clocks": clk.summary(), "gpu_launches": int(launches),
+            "parity_last_step": sampled_parity(torch, c, out, model=c.nmodel - 1, n=300)}
+    print(json.dumps(line), flush=True)
+
+
 def run_delens(args):
     """f1 measured alone: one step = lh_delens_grid over the whole grid for 80 sources (deflection planes resident)."""
     import torch
@@ -666,6 +705,9 @@ if __name__ == "__main__":
         raise SystemExit(0)
     if a.delens and a.impl != "reference":
         run_delens(a)
+        raise SystemExit(0)
+    if a.shared and a.impl != "reference":
+        run_shared(a)
         raise SystemExit(0)
     if a.impl == "reference":
         run_reference(a)
