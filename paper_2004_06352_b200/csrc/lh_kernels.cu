@@ -67,14 +67,14 @@ using SmemTables = MathTables;  // the atan / atanh reduction tables, staged per
 // vector register, and ptxas then gives up the uniform datapath for the whole record (vector LDC,
 // 3-register FMAs everywhere) -- measured, and guarded by tests/test_sass_cpu.py.
 template <bool GRAD, bool HESS>
-__device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Acc &a, const SmemTables &tb) {
+__device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Acc &a, const SmemTables &tb, const Consts &K) {
     const double dx = X - L.xc, dy = Y - L.yc;
     const double xp = fma(L.c, dx, L.s * dy);
     const double yp = fma(-L.s, dx, L.c * dy);
     const double xx = xp * xp, yy = yp * yp;
     const double vc = fma(L.ip, xx, L.im * yy) + L.rc2;  // k^2 (rc^2 + rho^2)
-    const double wc = sqrt_pos(vc);
-    const double wt = sqrt_pos(vc + L.dr2);  // k^2 (rt^2 + rho^2)
+    const double wc = sqrt_pos(vc, K);
+    const double wt = sqrt_pos(vc + L.dr2, K);  // k^2 (rt^2 + rho^2)
     const double Pc = wc + L.ac, Pt = wt + L.at;
     Reduced ra, rh;
     double Dc = 1.0, Dt = 1.0, i1, i2, fc, ft;
@@ -96,8 +96,8 @@ __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Ac
     else
         rcp2(wc * Dc, wt * Dt, fc, ft);
     if (GRAD) {
-        const double at = atan_finish(ra, i1, xp);
-        const double ah = atanh_finish(rh, i2, yp);
+        const double at = atan_finish(ra, i1, xp, K);
+        const double ah = atanh_finish(rh, i2, yp, K);
         a.ax = fma(L.cG, at, fma(-L.sG, ah, a.ax));
         a.ay = fma(L.sG, at, fma(L.cG, ah, a.ay));
     }
@@ -112,22 +112,22 @@ __device__ __forceinline__ void dpie_term(const LensK &L, double X, double Y, Ac
 
 // ---- NSIE: one PIEMD term ------------------------------------------------------------------
 template <bool GRAD, bool HESS>
-__device__ __forceinline__ void nsie_term(const LensK &L, double X, double Y, Acc &a, const SmemTables &tb) {
+__device__ __forceinline__ void nsie_term(const LensK &L, double X, double Y, Acc &a, const SmemTables &tb, const Consts &K) {
     const double dx = X - L.xc, dy = Y - L.yc;
     const double xp = fma(L.c, dx, L.s * dy);
     const double yp = fma(-L.s, dx, L.c * dy);
     const double xx = xp * xp, yy = yp * yp;
     const double rho2 = fma(L.ip, xx, L.im * yy);
     double wc, iwc;
-    rsqrt_sqrt(L.rc2 + rho2, wc, iwc);
+    rsqrt_sqrt(L.rc2 + rho2, wc, iwc, K);
     const double Pc = wc + L.ac;
     if (GRAD) {
         const Reduced ra = atan_reduce(fabs(xp), Pc, tb.at);
         const Reduced rh = atanh_reduce(fabs(yp), wc + L.bc, tb.ah);
         double i1, i2;
         rcp2(ra.den, rh.den, i1, i2);
-        const double at = atan_finish(ra, i1, xp);
-        const double ah = atanh_finish(rh, i2, yp);
+        const double at = atan_finish(ra, i1, xp, K);
+        const double ah = atanh_finish(rh, i2, yp, K);
         a.ax = fma(L.cG, at, fma(-L.sG, ah, a.ax));
         a.ay = fma(L.sG, at, fma(L.cG, ah, a.ay));
     }
@@ -188,11 +188,11 @@ __device__ __forceinline__ void extreme_term(const LensK &L, double X, double Y,
 
 // ---- SIS: alpha = b0 (dx,dy)/R, H = b0/R^3 [[dy^2,-dx dy],[-dx dy,dx^2]]; zero at R = 0 ---
 template <bool GRAD, bool HESS>
-__device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc &a) {
+__device__ __forceinline__ void sis_term(const LensK &L, double X, double Y, Acc &a, const Consts &K) {
     const double dx = X - L.xc, dy = Y - L.yc;
     const double R2 = fma(dx, dx, dy * dy);
     double R, iR;
-    rsqrt_sqrt(R2, R, iR);
+    rsqrt_sqrt(R2, R, iR, K);
     if (!(R2 > 0.0)) iR = 0.0;
     const double g = L.G * iR;
     if (GRAD) {
@@ -281,6 +281,7 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
     }
     __syncthreads();  // tables staged
 
+    const Consts K = P.kc;
     // class sub-ranges of this model's records (type-pure loops, no per-lens branch)
     const int b = m * P.stride;
     const int e0 = b + P.cls_end[m][0];  // end of dPIE
@@ -288,15 +289,15 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
     const int e2 = b + P.cls_end[m][2];  // end of SIS
     for (int l = b; l < e0; ++l) {
 #pragma unroll
-        for (int k = 0; k < PX; ++k) dpie_term<GRAD, HESS>(P.table[l], X[k], Yk[k], acc[k], tb);
+        for (int k = 0; k < PX; ++k) dpie_term<GRAD, HESS>(P.table[l], X[k], Yk[k], acc[k], tb, K);
     }
     for (int l = e0; l < e1; ++l) {
 #pragma unroll
-        for (int k = 0; k < PX; ++k) nsie_term<GRAD, HESS>(P.table[l], X[k], Yk[k], acc[k], tb);
+        for (int k = 0; k < PX; ++k) nsie_term<GRAD, HESS>(P.table[l], X[k], Yk[k], acc[k], tb, K);
     }
     for (int l = e1; l < e2; ++l) {
 #pragma unroll
-        for (int k = 0; k < PX; ++k) sis_term<GRAD, HESS>(P.table[l], X[k], Yk[k], acc[k]);
+        for (int k = 0; k < PX; ++k) sis_term<GRAD, HESS>(P.table[l], X[k], Yk[k], acc[k], K);
     }
     if (EXTREME) {
         const int e3 = b + P.cls_end[m][3];
@@ -423,6 +424,7 @@ static cudaError_t launch_one(const LaunchParams &P, dim3 grid, cudaStream_t str
 cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launches) {
     thread_local LaunchParams Q;  // 32 KB: kept off the stack
     Q.x0 = J.x0; Q.y0 = J.y0; Q.dx = J.dx;
+    Q.kc = Consts();
     Q.nx = J.nx; Q.ny = J.ny;
     Q.plane = J.plane;
     Q.j0 = J.j0;

@@ -14,6 +14,7 @@ constexpr int LAUNCH_MODELS = 160;  // models that may share one launch (blockId
 
 struct LaunchParams {
     double x0, y0, dx;
+    Consts kc;               // 1/3, 1/5, 3/8 as launch-parameter VALUES (lh_math.cuh: kept in registers, not rematerialised)
     long long plane;         // nx*ny
     double *out[9];          // ax ay a11 a12 a22 kappa gamma1 gamma2 mu; nullptr = not wanted; [nmodel][ny][nx]
     double *carry;           // [5][ny][nx] accumulators handed from one lens chunk of a model to the next

@@ -55,6 +55,15 @@ struct MathTables {
     double2 ah[LN_N];    // {c', atanh c'}, c' = 1 - t_c
 };
 
+// The three constants of the correction steps that have a non-zero low word or share an instruction with another
+// constant (an FP64 instruction takes ONE immediate / uniform operand, so the second constant needs a vector
+// register).  As literals ptxas rematerialises them inside the lens loop (two moves each per iteration, 8 in all);
+// the kernel therefore hands them in as VALUES it read from its launch parameters -- loop-invariant registers the
+// compiler cannot fold.  The defaults serve the host build and the stand-alone forms.
+struct Consts {
+    double third = 1.0 / 3.0, fifth = 0.2, c375 = 0.375;
+};
+
 // ---- bit access -------------------------------------------------------------------------------
 LH_HD int hi32(double x) {
 #ifdef __CUDA_ARCH__
@@ -124,21 +133,21 @@ LH_HD void rcp4(double a, double b, double c, double d, double &ia, double &ib, 
 //   (1 + h) y and (1 + h) v y,  h = e (1/2 + 3 e/8), e = 1 - v y^2.     6 FP64 + 1 MUFU
 // (both closing FMAs read one register twice: two distinct registers each; a caller that
 // drops iw pays 5)
-LH_HD void rsqrt_sqrt(double v, double &w, double &iw) {
+LH_HD void rsqrt_sqrt(double v, double &w, double &iw, const Consts &K = Consts()) {
     const double y = rsq_seed(v);
     const double t = v * y;
     const double e = fma(-t, y, 1.0);
-    const double h = fma(0.375, e, 0.5) * e;
+    const double h = fma(K.c375, e, 0.5) * e;
     iw = fma(y, h, y);
     w = fma(t, h, t);
 }
 
 // w = sqrt(v) alone (same seed and step as rsqrt_sqrt, without the closing FMA of 1/sqrt).   5 FP64 + 1 MUFU
-LH_HD double sqrt_pos(double v) {
+LH_HD double sqrt_pos(double v, const Consts &K = Consts()) {
     const double y = rsq_seed(v);
     const double t = v * y;
     const double e = fma(-t, y, 1.0);
-    const double h = fma(0.375, e, 0.5) * e;
+    const double h = fma(K.c375, e, 0.5) * e;
     return fma(t, h, t);
 }
 
@@ -185,10 +194,10 @@ LH_HD Reduced atan_reduce(double an, double d, const double2 *__restrict__ tab) 
     const double2 ca = tab[quot_index_up(qp, ATAN_N)];
     return Reduced{fma(-ca.x, d, an), fma(ca.x, an, d), ca.y};
 }
-LH_HD double atan_finish(const Reduced &r, double iden, double sgn) {
+LH_HD double atan_finish(const Reduced &r, double iden, double sgn, const Consts &K = Consts()) {
     const double z = r.num * iden;  // |z| <= 2^-8
     const double z2 = z * z;
-    const double p = fma(z2, fma(z2, 0.2, -1.0 / 3.0), 1.0);
+    const double p = fma(z2, fma(z2, K.fifth, -K.third), 1.0);
     return copysign_pos_i(fma(z, p, r.base), sgn);
 }
 
@@ -208,10 +217,10 @@ LH_HD Reduced atanh_reduce(double an, double d, const double2 *__restrict__ tab)
     const double2 ca = tab[quot_index_down(t0, LN_N)];
     return Reduced{fma(-ca.x, d, an), fma(-ca.x, an, d), ca.y};
 }
-LH_HD double atanh_finish(const Reduced &r, double iden, double sgn) {
+LH_HD double atanh_finish(const Reduced &r, double iden, double sgn, const Consts &K = Consts()) {
     const double s = r.num * iden;
     const double s2 = s * s;
-    const double p = fma(s2, fma(s2, 0.2, 1.0 / 3.0), 1.0);
+    const double p = fma(s2, fma(s2, K.fifth, K.third), 1.0);
     return copysign_pos_i(fma(s, p, r.base), sgn);
 }
 
