@@ -69,6 +69,10 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scaling", default="auto", choices=["auto", "strong", "weak"],
                     help="N > 1: strong = row slabs of ONE map (default), weak = an independent lens model per rank")
+    ap.add_argument("--assemble", default="auto", choices=["auto", "peer", "gather"],
+                    help="strong scaling: how the one map reaches rank 0 -- peer: every rank's kernel stores its rows straight "
+                         "into rank 0's planes (CUDA IPC + NVLink peer access, no second pass); gather: one dist.gather "
+                         "after the computation; auto: peer when the mapping succeeds on every rank, else gather")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="target CPU time of the all-cores oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -361,12 +365,41 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     lh.lh_set_stream(stream)
 
+    # ---- strong scaling, peer mode: rank 0 owns the one map; every other rank maps it (CUDA IPC) and its kernel
+    # stores its rows straight into it -- the assembly rides on the epilogue stores, no gather, no second pass
+    peer, peer_ptrs, owner_map = None, {}, None
+    if scaling == "strong" and world > 1 and args.assemble in ("auto", "peer"):
+        ok, err = 1, ""
+        try:
+            if rank == 0:
+                owner_map = {n: torch.empty((g.ny, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs}
+                handles = [{n: lh.lh_ipc_export(t) for n, t in owner_map.items()}]
+            else:
+                handles = [None]
+            dist.broadcast_object_list(handles, src=0)
+            if rank == 0:
+                peer = {n: owner_map[n][j0:j0 + nrows] for n in cfg.outputs}
+            else:
+                for n in cfg.outputs:
+                    peer_ptrs[n] = lh.lh_ipc_open(*handles[0][n])
+                peer = {n: peer_ptrs[n] + j0 * g.nx * 8 for n in cfg.outputs}  # address of this rank's first row
+        except Exception as e:  # no IPC / no peer access on this machine: fall back to the gather
+            ok, err = 0, repr(e)
+        t = torch.tensor([float(ok)], dtype=torch.float64, device=red_dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MIN)
+        if float(t.item()) < 1.0:
+            if args.assemble == "peer":
+                raise SystemExit(f"--assemble peer: the owner's map could not be mapped on every rank ({err})")
+            for ptr in peer_ptrs.values():
+                lh.lh_ipc_close(ptr)
+            peer, peer_ptrs, owner_map = None, {}, None
+
     def step():
         if args.stats:
             lh.lh_grid_stats_batch(lenses, cfg.nmodel, cfg.nlens, g, out, var)
         elif scaling == "strong":
             if nrows > 0:
-                lh.lh_grid_eval_rows(lenses, g, j0, nrows, **out)
+                lh.lh_grid_eval_rows(lenses, g, j0, nrows, **(peer if peer is not None else out))
         else:
             lh.lh_grid_eval_batch(lenses, cfg.nmodel, cfg.nlens, g, **out)
 
@@ -391,9 +424,28 @@ def run_ours(args):
     job_evals = cfg.evals * (world if scaling == "weak" else 1)  # units ALL ranks processed per step
     value = job_evals / (ms_per_step * 1e-3)
 
-    # ---- strong scaling: the time to assemble the one map on rank 0 (not part of the computation)
+    # ---- strong scaling, peer mode: the timed steps already left the whole map in rank 0's planes
     assemble = None
-    if scaling == "strong" and world > 1:
+    if peer is not None:
+        if nrows > 0:
+            lh.lh_grid_eval_rows(lenses, g, j0, nrows, **out)  # this rank's own copy (parity sample, e2e comparison)
+        barrier()  # every writer synchronised: the owner may read
+        assemble = {"ms": 0.0, "bytes": int(len(cfg.outputs) * g.npix * 8), "mode": "peer",
+                    "how": "every rank's lh_grid_eval_rows stores its rows straight into rank 0's planes (CUDA IPC mapping, "
+                           "peer access over NVLink): the assembly is inside the timed steps, no gather, no second pass",
+                    "bitwise_check": None}
+        if rank == 0:
+            ref = {n: torch.empty((g.ny, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs}
+            lh.lh_grid_eval(lenses, g, **ref)
+            torch.cuda.synchronize()
+            assemble["bitwise_check"] = all(bool((owner_map[n].view(torch.int64) == ref[n].view(torch.int64)).all())
+                                            for n in cfg.outputs)
+            del ref
+        barrier()
+        for ptr in peer_ptrs.values():
+            lh.lh_ipc_close(ptr)
+    # ---- strong scaling, gather mode: the time to assemble the one map on rank 0 (not part of the computation)
+    if scaling == "strong" and world > 1 and peer is None:
         rows_of = [li.row_slab(g, r, world)[1] for r in range(world)]
         pad = max(rows_of)
         full = {n: torch.empty((world, pad, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs} if rank == 0 else None
@@ -423,7 +475,7 @@ def run_ours(args):
         dev_ms = reduce_max(e0.elapsed_time(e1) / 3)
         wall_ms = reduce_max((time.perf_counter() - t0) * 1e3 / 3)
         assemble = {"ms": dev_ms if backend == "nccl" else wall_ms, "bytes": int(len(cfg.outputs) * g.npix * 8),
-                    "how": ("one dist.gather (NCCL) of every rank's slab of each plane into rank 0's map, CUDA events, "
+                    "mode": "gather", "how": ("one dist.gather (NCCL) of every rank's slab of each plane into rank 0's map, CUDA events, "
                             "max over ranks" if backend == "nccl" else "gloo stand-in through host memory, wall clock"),
                     "bitwise_check": None}
         if rank == 0:  # the assembled map is the single-device map, bit for bit (checked on rank 0's own device)

@@ -259,6 +259,26 @@ int lh_fp64_peak_probe(int iters, double *flops_per_s, double *seconds);
  * No CUDA call is made.  LH_EINVAL for an unknown fn or a NULL pointer (b may be NULL for fn 0-2). */
 int lh_math_host_eval(int fn, const double *a, const double *b, size_t n, double *out);
 
+/* ---- several GPUs, one process each: writing a row slab straight into the owner's map ----
+ * The output planes of lh_grid_eval_rows are plain device pointers, so a rank may hand it the address of ITS rows
+ * inside a map that lives on ANOTHER device: the kernel's epilogue stores then travel over NVLink (peer access) while
+ * the rest of the grid is still computing, and the one map is assembled with no gather and no second pass
+ * (PAPER.md:194 "the grid is split among the GPUs"; pixels are independent, :175).  Across processes the owner's buffer
+ * is reached through CUDA IPC; these three calls are thin wrappers of cudaIpcGetMemHandle / cudaIpcOpenMemHandle /
+ * cudaIpcCloseMemHandle that also deal with a buffer sitting inside a larger allocation (a caching allocator's).
+ *   lh_ipc_export  `dev_ptr`: device memory of THIS process.  Writes the 64-byte handle of the allocation that holds
+ *                  it and the byte offset of `dev_ptr` inside that allocation.
+ *   lh_ipc_open    maps the exporter's allocation into this process (another process than the exporter) and returns
+ *                  the address that corresponds to the exported `dev_ptr`.  The exporter's device must be the current
+ *                  one or peer-accessible from it.
+ *   lh_ipc_close   unmaps it (the pointer lh_ipc_open returned).
+ * Ordering is the caller's: the owner may read its map once every writer's stream has been synchronised (e.g. a
+ * barrier after torch.cuda.synchronize()).  LH_EINVAL: NULL argument, unknown pointer; LH_ECUDA: a CUDA call failed. */
+#define LH_IPC_HANDLE_BYTES 64
+int lh_ipc_export(const void *dev_ptr, unsigned char handle[LH_IPC_HANDLE_BYTES], unsigned long long *offset);
+int lh_ipc_open(const unsigned char handle[LH_IPC_HANDLE_BYTES], unsigned long long offset, void **dev_ptr);
+int lh_ipc_close(void *dev_ptr);
+
 /* "lh <major>.<minor> sm_100a" */
 const char *lh_version(void);
 

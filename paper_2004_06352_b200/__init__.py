@@ -8,7 +8,8 @@ missing -- there is no CPU fallback (and it never imports `oracle`).
 Names mirror the C ABI one to one:
     lh_grid_gradient, lh_grid_hessian, lh_lens_maps, lh_grid_gradient_batch,
     lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_grid_eval_rows_host, lh_grid_stats_batch, lh_pack_model, lh_set_stream,
-    lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_math_host_eval, lh_version
+    lh_ipc_export, lh_ipc_open, lh_ipc_close, lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_math_host_eval,
+    lh_version
 Outputs may be torch CUDA tensors (float64, contiguous), anything with a
 `data_ptr()`, or raw integer device addresses.
 """
@@ -85,6 +86,12 @@ def _load():
         L.lh_delens_grid.argtypes = [dp, dp, gp, vp, ci, vp, C.c_longlong, vp]
         L.lh_delens_grid.restype = ci
         L.lh_set_stream.argtypes = [vp]
+        L.lh_ipc_export.argtypes = [vp, vp, C.POINTER(C.c_ulonglong)]
+        L.lh_ipc_export.restype = ci
+        L.lh_ipc_open.argtypes = [vp, C.c_ulonglong, C.POINTER(vp)]
+        L.lh_ipc_open.restype = ci
+        L.lh_ipc_close.argtypes = [vp]
+        L.lh_ipc_close.restype = ci
         L.lh_pack_model.argtypes = [vp, ci, vp, vp]
         L.lh_pack_model.restype = ci
         L.lh_last_error.restype = C.c_char_p
@@ -325,6 +332,28 @@ def lh_pack_model(lenses, validate_only: bool = False):
     table = raw[off: off + n * LH_PACK_DOUBLES]
     _check(_load().lh_pack_model(p, n, table.ctypes.data, begin.ctypes.data))
     return table.reshape(n, LH_PACK_DOUBLES), begin
+
+
+def lh_ipc_export(t):
+    """(handle bytes, offset) of a device tensor / address of this process, for lh_ipc_open in another process."""
+    h = (C.c_ubyte * 64)()
+    off = C.c_ulonglong(0)
+    p = t if isinstance(t, int) else t.data_ptr()
+    _check(_load().lh_ipc_export(p, h, C.byref(off)))
+    return bytes(h), int(off.value)
+
+
+def lh_ipc_open(handle: bytes, offset: int) -> int:
+    """Device address, in THIS process, of the buffer another process exported (peer access over NVLink when it
+    lives on another GPU).  Pass it (plus a byte offset) as an output plane; close it with lh_ipc_close."""
+    h = (C.c_ubyte * 64).from_buffer_copy(handle)
+    out = C.c_void_p()
+    _check(_load().lh_ipc_open(h, int(offset), C.byref(out)))
+    return int(out.value)
+
+
+def lh_ipc_close(ptr: int) -> None:
+    _check(_load().lh_ipc_close(int(ptr)))
 
 
 def lh_set_stream(stream) -> None:

@@ -696,6 +696,66 @@ int lh_pack_model(const lh_lens *lenses, int n, double *table, int32_t *class_be
     return LH_OK;
 }
 
+// ---- CUDA IPC wrappers (include/lh.h: a rank's slab written straight into the owner's map) -----------------------
+namespace {
+struct IpcMapping { void *user; void *base; };
+std::mutex ipc_mu;
+std::vector<IpcMapping> ipc_open_list;
+}  // namespace
+
+int lh_ipc_export(const void *dev_ptr, unsigned char handle[LH_IPC_HANDLE_BYTES], unsigned long long *offset) {
+    static_assert(sizeof(cudaIpcMemHandle_t) == LH_IPC_HANDLE_BYTES, "lh.h out of date");
+    ctx.err[0] = 0;
+    if (!dev_ptr || !handle || !offset) return fail(LH_EINVAL, "lh_ipc_export: NULL argument");
+    int rc = check_device_ptr(static_cast<const double *>(dev_ptr), "dev_ptr");
+    if (rc) return rc;
+    // base of the allocation that holds dev_ptr (driver entry point fetched at run time: no link-time libcuda)
+    typedef int (*range_fn)(unsigned long long *, size_t *, unsigned long long);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    CU(cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &qr));
+    if (!fn || qr != cudaDriverEntryPointSuccess) return fail(LH_ECUDA, "cuMemGetAddressRange is not available");
+    unsigned long long base = 0;
+    size_t size = 0;
+    if (reinterpret_cast<range_fn>(fn)(&base, &size, (unsigned long long)reinterpret_cast<uintptr_t>(dev_ptr)) != 0)
+        return fail(LH_EINVAL, "lh_ipc_export: not the address of a device allocation");
+    cudaIpcMemHandle_t h;
+    CU(cudaIpcGetMemHandle(&h, reinterpret_cast<void *>(static_cast<uintptr_t>(base))));
+    std::memcpy(handle, &h, sizeof(h));
+    *offset = (unsigned long long)reinterpret_cast<uintptr_t>(dev_ptr) - base;
+    return LH_OK;
+}
+
+int lh_ipc_open(const unsigned char handle[LH_IPC_HANDLE_BYTES], unsigned long long offset, void **dev_ptr) {
+    ctx.err[0] = 0;
+    if (!handle || !dev_ptr) return fail(LH_EINVAL, "lh_ipc_open: NULL argument");
+    cudaIpcMemHandle_t h;
+    std::memcpy(&h, handle, sizeof(h));
+    void *base = nullptr;
+    CU(cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
+    *dev_ptr = static_cast<char *>(base) + offset;
+    std::lock_guard<std::mutex> lock(ipc_mu);
+    ipc_open_list.push_back(IpcMapping{*dev_ptr, base});
+    return LH_OK;
+}
+
+int lh_ipc_close(void *dev_ptr) {
+    ctx.err[0] = 0;
+    void *base = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(ipc_mu);
+        for (size_t k = 0; k < ipc_open_list.size(); ++k)
+            if (ipc_open_list[k].user == dev_ptr) {
+                base = ipc_open_list[k].base;
+                ipc_open_list.erase(ipc_open_list.begin() + (long)k);
+                break;
+            }
+    }
+    if (!base) return fail(LH_EINVAL, "lh_ipc_close: not a pointer lh_ipc_open returned");
+    CU(cudaIpcCloseMemHandle(base));
+    return LH_OK;
+}
+
 int lh_set_stream(void *cuda_stream) {
     ctx.stream = static_cast<cudaStream_t>(cuda_stream);
     return LH_OK;

@@ -592,10 +592,13 @@ def test_two_devices_row_slabs_assemble_the_single_device_map_bitwise():
         assert torch.equal(asm[n].view(torch.int64), full[n].view(torch.int64))
 
 
-def test_bench_strong_scaling_arm_two_ranks_over_gloo():
+@pytest.mark.parametrize("assemble", ["peer", "gather"])
+def test_bench_strong_scaling_arm_two_ranks_over_gloo(assemble):
     """`bench.py --gpus 2` as the driver launches it (torchrun, one process per rank), with the process group on gloo
     so that two ranks can share this one GPU: the default N > 1 arm shards the ROWS of one map, the
-    assembled map equals the single-device map bit for bit, and the line carries the contract's keys."""
+    assembled map equals the single-device map bit for bit, and the line carries the contract's keys.  `peer`: rank 1
+    maps rank 0's planes through CUDA IPC and its kernel stores its rows straight into them (on several GPUs the
+    same stores cross NVLink); `gather`: one gather after the computation."""
     import json
     import socket
     import subprocess
@@ -608,14 +611,52 @@ def test_bench_strong_scaling_arm_two_ranks_over_gloo():
     env = dict(os.environ, LH_BENCH_BACKEND="gloo")
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
            "127.0.0.1", "--master-port", str(port), os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "3",
-           "--warmup", "3", "--config", "1", "--no-cpu-baseline"]
+           "--warmup", "3", "--config", "1", "--no-cpu-baseline", "--assemble", assemble]
     r = subprocess.run(cmd, env=env, cwd=root, capture_output=True, text=True, timeout=600)
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
     assert len(lines) == 1, r.stdout[-2000:]
     d = json.loads(lines[0])
     assert d["n_gpus"] == 2 and d["scaling"] == "strong" and d["gpu_launches"] == 3  # rank 0: one launch per step
+    assert d["assemble"]["mode"] == assemble
     assert d["assemble"]["bitwise_check"] is True and d["assemble"]["bytes"] == 2 * 1024 * 1024 * 8
     assert d["parity_last_step"]["ok"] and d["e2e"]["same_bits_as_device_planes"] is True
     assert d["config"]["evals_per_step"] == 1024 * 1024 * 100
     assert abs(d["value"] - d["config"]["evals_per_step"] / (d["ms_per_step"] * 1e-3)) < 1e-6 * d["value"]
+
+
+def test_ipc_export_open_roundtrip_in_another_process():
+    """lh_ipc_export / lh_ipc_open / lh_ipc_close: a child process maps a tensor of this process (which sits INSIDE a
+    larger allocation of torch's caching allocator, at a non-zero offset), lets lh_grid_eval_rows write two rows of
+    a map into it through the mapped address, and this process finds exactly those rows written."""
+    import subprocess
+    import sys
+
+    c = li.config(1, scale=8)
+    g = c.grid
+    pad = torch.empty(12345, dtype=torch.float64, device="cuda")  # pushes the next tensor off the segment start
+    buf = torch.full((g.ny, g.nx), float("nan"), dtype=torch.float64, device="cuda")
+    handle, offset = lh.lh_ipc_export(buf)
+    torch.cuda.synchronize()
+    child = f"""
+import sys, numpy as np
+sys.path.insert(0, {os.path.dirname(os.path.dirname(os.path.abspath(__file__)))!r})
+import torch, lens_inputs as li, paper_2004_06352_b200 as lh
+torch.cuda.set_device(0)
+c = li.config(1, scale=8); g = c.grid
+p = lh.lh_ipc_open(bytes.fromhex({handle.hex()!r}), {offset})
+lh.lh_grid_eval_rows(c.lenses, g, 5, 2, ax=p + 5 * g.nx * 8)
+torch.cuda.synchronize()
+lh.lh_ipc_close(p)
+try:
+    lh.lh_ipc_close(p)
+except lh.LhError:
+    print("second close refused")
+"""
+    r = subprocess.run([sys.executable, "-c", child], capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0 and "second close refused" in r.stdout, r.stderr[-2000:]
+    torch.cuda.synchronize()
+    ref = run_gpu(c.lenses, g, ("ax",))["ax"]
+    got = buf.cpu().numpy()
+    assert np.array_equal(got[5:7], ref[5:7]) and np.isnan(got[:5]).all() and np.isnan(got[7:]).all()
+    del pad
