@@ -166,3 +166,32 @@ def test_binding_checks_host_plane_sizes_before_the_call():
         lh.lh_grid_eval_host(np.concatenate([c.lenses, c.lenses]), 2, c.nlens, g, ax=np.empty(g.npix))
     with pytest.raises(TypeError):
         lh.lh_grid_eval_host(c.lenses, 1, c.nlens, g, ax=np.empty(g.npix, dtype=np.float32))
+
+
+def test_row_slab_and_ipc_argument_errors_before_any_cuda_work():
+    """lh_grid_eval_rows / lh_grid_eval_rows_host: a slab outside the grid; the IPC wrappers: NULL / unknown pointers."""
+    c = li.config(0)
+    g = c.grid
+    for j0, nrows in ((-1, 2), (0, 0), (g.ny - 1, 2), (g.ny, 1)):
+        with pytest.raises(lh.LhError) as e:
+            lh.lh_grid_eval_rows(c.lenses, g, j0, nrows, ax=256)
+        assert e.value.code == lh.LH_EINVAL and "slab" in str(e.value)
+        with pytest.raises(lh.LhError) as e:
+            lh.lh_grid_eval_rows_host(c.lenses, g, j0, nrows, ax=np.empty(max(nrows, 1) * g.nx))
+        assert e.value.code == lh.LH_EINVAL and "slab" in str(e.value)
+    with pytest.raises(lh.LhError) as e:  # a bad lens is reported before anything else happens
+        bad = c.lenses.copy()
+        bad["rcut"][2] = 0.0
+        lh.lh_grid_eval_rows_host(bad, g, 0, 4, ax=np.empty(4 * g.nx))
+    assert e.value.code == lh.LH_EINVAL and "lens 2" in str(e.value)
+    with pytest.raises(lh.LhError) as e:
+        lh.lh_ipc_export(0)
+    assert e.value.code == lh.LH_EINVAL
+    buf = np.zeros(16)
+    with pytest.raises(lh.LhError) as e:  # host memory cannot be exported
+        lh.lh_ipc_export(buf.ctypes.data)
+    assert e.value.code == lh.LH_EINVAL
+    with pytest.raises(lh.LhError) as e:
+        lh.lh_ipc_close(12345 * 8)
+    assert e.value.code == lh.LH_EINVAL
+    assert lh.lh_launch_count() == 0
