@@ -24,6 +24,22 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+LIB_CHECK = os.path.join(HERE, "liblh_check.so")
+
+
+def build_check(force: bool = False) -> str:
+    """The CHECKING build of the same sources (-DLH_BOUNDS_CHECK): every global-memory access of the superposition kernel
+    is compared with the address ranges the launch was given; a stand-in for compute-sanitizer memcheck, which is
+    closed on this GPU pool.  Test infrastructure (tests/test_gpu_bounds.py); never loaded by the product path."""
+    stale = not os.path.exists(LIB_CHECK) or any(
+        os.path.getmtime(os.path.join(CSRC, f)) > os.path.getmtime(LIB_CHECK) for f in SOURCES + HEADERS)
+    if force or stale:
+        nvcc = os.environ.get("NVCC", "nvcc")
+        cmd = [nvcc, *NVCC_FLAGS, "-DLH_BOUNDS_CHECK", "-o", LIB_CHECK] + [os.path.join(CSRC, s) for s in SOURCES]
+        subprocess.run(cmd, check=True, cwd=CSRC)
+    return LIB_CHECK
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "nvcc")

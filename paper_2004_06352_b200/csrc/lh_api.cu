@@ -81,6 +81,16 @@ struct Context {
 
 thread_local Context ctx;
 
+#ifdef LH_BOUNDS_CHECK
+// Checking build only (liblh_check.so): the address ranges the caller allows superpose_kernel to touch
+// (lh_debug_bounds_add) and the device counter of refused accesses.  Test infrastructure: one host thread.
+struct DebugBounds {
+    const char *lo[lh::DBG_RANGES], *hi[lh::DBG_RANGES];
+    int n = 0;
+    unsigned long long *d_count = nullptr;
+} dbg;
+#endif
+
 // state of the device that is current on this host thread
 DeviceState &DS() {
     int d = 0;
@@ -274,6 +284,25 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
         J.ev_join = DS().ev_join;
         if (stats_scratch) J.stats_scratch = DS().d_carry + 2 * (carry_one / sizeof(double));
     }
+#ifdef LH_BOUNDS_CHECK
+    if (!dbg.d_count) {
+        CU(cudaMalloc(&dbg.d_count, sizeof(unsigned long long)));
+        CU(cudaMemset(dbg.d_count, 0, sizeof(unsigned long long)));
+    }
+    J.dbg_count = dbg.d_count;
+    J.dbg_n = 0;
+    for (int r = 0; r < dbg.n; ++r) { J.dbg_lo[J.dbg_n] = dbg.lo[r]; J.dbg_hi[J.dbg_n] = dbg.hi[r]; ++J.dbg_n; }
+    // the library's own buffers: the carry / statistics scratch exactly as large as THIS job needs it (the cached
+    // allocation may be larger), and the reduction tables
+    if (carry_need) {
+        J.dbg_lo[J.dbg_n] = reinterpret_cast<const char *>(DS().d_carry);
+        J.dbg_hi[J.dbg_n] = reinterpret_cast<const char *>(DS().d_carry) + carry_need;
+        ++J.dbg_n;
+    }
+    J.dbg_lo[J.dbg_n] = reinterpret_cast<const char *>(J.math);
+    J.dbg_hi[J.dbg_n] = reinterpret_cast<const char *>(J.math) + sizeof(lh::MathTables);
+    ++J.dbg_n;
+#endif
     CU(lh::launch_eval(J, s, &ctx.launches));
     if (carry_need) {
         CU(cudaEventRecord(DS().ev_done, s));
@@ -627,6 +656,14 @@ int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, in
     int slot = 0;
     for (int k = 0; k < NPLANES; ++k)
         dp[k] = hp[k] ? DS().d_planes + (size_t)(slot++) * (plane_bytes / sizeof(double)) : nullptr;
+#ifdef LH_BOUNDS_CHECK
+    // the internal device planes of this call, exactly as large as the call needs them (popped again below)
+    struct PopRange { ~PopRange() { --dbg.n; } } pop_range;
+    if (dbg.n >= lh::DBG_RANGES - 2) { ++dbg.n; return fail(LH_EINVAL, "too many debug ranges"); }
+    dbg.lo[dbg.n] = reinterpret_cast<const char *>(DS().d_planes);
+    dbg.hi[dbg.n] = reinterpret_cast<const char *>(DS().d_planes) + need;
+    ++dbg.n;
+#endif
 
     // Pipeline: the work is cut into pieces (row slabs of one map, or groups of models of a batch); the
     // device-to-host copy of piece k runs on a second stream while piece k+1 is being computed.
@@ -755,6 +792,32 @@ int lh_ipc_close(void *dev_ptr) {
     CU(cudaIpcCloseMemHandle(base));
     return LH_OK;
 }
+
+#ifdef LH_BOUNDS_CHECK
+// ---- checking build only; not declared in include/lh.h (tests/test_gpu_bounds.py declares them itself) -------------
+int lh_debug_bounds_reset(void) {
+    dbg.n = 0;
+    if (dbg.d_count) {
+        CU(cudaDeviceSynchronize());
+        CU(cudaMemset(dbg.d_count, 0, sizeof(unsigned long long)));
+    }
+    return LH_OK;
+}
+int lh_debug_bounds_add(const void *p, unsigned long long bytes) {
+    if (!p || dbg.n >= lh::DBG_RANGES - 2) return fail(LH_EINVAL, "lh_debug_bounds_add: NULL or too many ranges");
+    dbg.lo[dbg.n] = static_cast<const char *>(p);
+    dbg.hi[dbg.n] = static_cast<const char *>(p) + bytes;
+    ++dbg.n;
+    return LH_OK;
+}
+long long lh_debug_violations(void) {
+    if (!dbg.d_count) return 0;
+    unsigned long long v = 0;
+    if (cudaDeviceSynchronize() != cudaSuccess) return -1;
+    if (cudaMemcpy(&v, dbg.d_count, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+    return (long long)v;
+}
+#endif
 
 int lh_set_stream(void *cuda_stream) {
     ctx.stream = static_cast<cudaStream_t>(cuda_stream);

@@ -51,6 +51,31 @@ struct Acc {
     double ax, ay, S, Dl, a12;
 };
 
+// ---- checking build (-DLH_BOUNDS_CHECK, liblh_check.so; tests/test_gpu_bounds.py) -----------------------------
+// compute-sanitizer is closed on this GPU pool (profiles/r02_sanitizer.md), so the kernel can check itself: every
+// global-memory access of superpose_kernel goes through LD / ST, which in the checking build compare the address
+// with the list of ranges the launch was given (the caller's buffers, registered through lh_debug_bounds_add, and
+// the library's own carry / statistics / table buffers), count a violation and SKIP the access instead of making it.
+// In the product build they are the plain access.
+#ifdef LH_BOUNDS_CHECK
+__device__ __forceinline__ bool dbg_ok(const LaunchParams &P, const void *p, unsigned bytes) {
+    const char *a = static_cast<const char *>(p);
+    for (int r = 0; r < P.dbg_n; ++r)
+        if (a >= P.dbg_lo[r] && a + bytes <= P.dbg_hi[r]) return true;
+    atomicAdd(P.dbg_count, 1ULL);
+    return false;
+}
+#define LH_LD(p) (dbg_ok(P, (p), 8) ? *(p) : 0.0)
+#define LH_LDG(p) (dbg_ok(P, (p), sizeof(*(p))) ? __ldg(p) : decltype(__ldg(p))())
+#define LH_ST(p, v) do { if (dbg_ok(P, (p), 8)) *(p) = (v); } while (0)
+#define LH_ST2(p, v) do { if (dbg_ok(P, (p), 16)) *(p) = (v); } while (0)
+#else
+#define LH_LD(p) (*(p))
+#define LH_LDG(p) __ldg(p)
+#define LH_ST(p, v) (*(p) = (v))
+#define LH_ST2(p, v) (*(p) = (v))
+#endif
+
 using SmemTables = MathTables;  // the atan / atanh reduction tables, staged per CTA
 
 // ---- dPIE: core term minus cut term, merged ---------------------
@@ -234,7 +259,7 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
     {
         const double2 *src = reinterpret_cast<const double2 *>(P.math);
         double2 *dst = reinterpret_cast<double2 *>(&tb);
-        for (int t = threadIdx.x; t < (int)(sizeof(SmemTables) / sizeof(double2)); t += THREADS) dst[t] = __ldg(src + t);
+        for (int t = threadIdx.x; t < (int)(sizeof(SmemTables) / sizeof(double2)); t += THREADS) dst[t] = LH_LDG(src + t);
     }
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -254,8 +279,8 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
     for (int k = 0; k < PX; ++k) {
         if (POINTS) {
             const bool in = inside && i0 + k < P.nx;
-            X[k] = in ? __ldg(P.px + i0 + k) : 0.0;
-            Yk[k] = in ? __ldg(P.py + i0 + k) : 0.0;
+            X[k] = in ? LH_LDG(P.px + i0 + k) : 0.0;
+            Yk[k] = in ? LH_LDG(P.py + i0 + k) : 0.0;
         } else {
             X[k] = __dadd_rn(P.x0, __dmul_rn((double)(i0 + k), P.dx));
             Yk[k] = Y;
@@ -274,8 +299,8 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
         for (int k = 0; k < PX; ++k) {
             if (i0 + k < P.nx) {
                 const double *c = P.carry + pix + k;
-                if (GRAD) { acc[k].ax = c[0]; acc[k].ay = c[P.plane]; }
-                if (HESS) { acc[k].S = c[2 * P.plane]; acc[k].Dl = c[3 * P.plane]; acc[k].a12 = c[4 * P.plane]; }
+                if (GRAD) { acc[k].ax = LH_LD(c); acc[k].ay = LH_LD(c + P.plane); }
+                if (HESS) { acc[k].S = LH_LD(c + 2 * P.plane); acc[k].Dl = LH_LD(c + 3 * P.plane); acc[k].a12 = LH_LD(c + 4 * P.plane); }
             }
         }
     }
@@ -313,8 +338,8 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
         for (int k = 0; k < PX; ++k) {
             if (i0 + k < P.nx) {
                 double *c = P.carry + pix + k;
-                if (GRAD) { c[0] = acc[k].ax; c[P.plane] = acc[k].ay; }
-                if (HESS) { c[2 * P.plane] = acc[k].S; c[3 * P.plane] = acc[k].Dl; c[4 * P.plane] = acc[k].a12; }
+                if (GRAD) { LH_ST(c, acc[k].ax); LH_ST(c + P.plane, acc[k].ay); }
+                if (HESS) { LH_ST(c + 2 * P.plane, acc[k].S); LH_ST(c + 3 * P.plane, acc[k].Dl); LH_ST(c + 4 * P.plane, acc[k].a12); }
             }
         }
         return;
@@ -354,15 +379,15 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
                 if (i0 + k >= P.nx) continue;
                 double mean = 0.0, m2 = 0.0;
                 if (P.stats_n > 1) {
-                    mean = o[pix + k];
-                    if (q) m2 = q[pix + k];
+                    mean = LH_LD(o + pix + k);
+                    if (q) m2 = LH_LD(q + pix + k);
                 }
                 const double d = v[pl][k] - mean;
                 mean += d / n;
-                o[pix + k] = mean;
+                LH_ST(o + pix + k, mean);
                 if (q) {
                     m2 = fma(d, v[pl][k] - mean, m2);
-                    q[pix + k] = (P.stats == 2) ? m2 / n : m2;
+                    LH_ST(q + pix + k, (P.stats == 2) ? m2 / n : m2);
                 }
             }
         }
@@ -377,10 +402,10 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
 #pragma unroll
         for (int k = 0; k < PX; k += 2) {
             if (al && i0 + k + 1 < P.nx) {
-                *reinterpret_cast<double2 *>(o + idx + k) = make_double2(v[pl][k], v[pl][k + 1]);
+                LH_ST2(reinterpret_cast<double2 *>(o + idx + k), make_double2(v[pl][k], v[pl][k + 1]));
             } else {
-                if (i0 + k < P.nx) o[idx + k] = v[pl][k];
-                if (i0 + k + 1 < P.nx) o[idx + k + 1] = v[pl][k + 1];
+                if (i0 + k < P.nx) LH_ST(o + idx + k, v[pl][k]);
+                if (i0 + k + 1 < P.nx) LH_ST(o + idx + k + 1, v[pl][k + 1]);
             }
         }
     }
@@ -425,6 +450,10 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     thread_local LaunchParams Q;  // 32 KB: kept off the stack
     Q.x0 = J.x0; Q.y0 = J.y0; Q.dx = J.dx;
     Q.kc = Consts();
+#ifdef LH_BOUNDS_CHECK
+    Q.dbg_n = J.dbg_n; Q.dbg_count = J.dbg_count;
+    for (int r = 0; r < J.dbg_n; ++r) { Q.dbg_lo[r] = J.dbg_lo[r]; Q.dbg_hi[r] = J.dbg_hi[r]; }
+#endif
     Q.nx = J.nx; Q.ny = J.ny;
     Q.plane = J.plane;
     Q.j0 = J.j0;

@@ -11,6 +11,7 @@ namespace lh {
 // 160 x 192 B of lens constants + 160 x 8 B of class boundaries + a header of about 250 bytes.
 constexpr int LAUNCH_RECORDS = 160;
 constexpr int LAUNCH_MODELS = 160;  // models that may share one launch (blockIdx.y)
+constexpr int DBG_RANGES = 16;      // checking build (-DLH_BOUNDS_CHECK): address ranges a launch may touch
 
 struct LaunchParams {
     double x0, y0, dx;
@@ -29,6 +30,11 @@ struct LaunchParams {
                              // running sums of squared deviations (Welford); 2 = last model: m2[] is divided by the count
     double *m2[9];           // stats only; nullptr = variance of that plane not wanted
     const double *px, *py;   // POINTS variants only: coordinates of "pixel" i (then ny = 1, nx = number of points)
+#ifdef LH_BOUNDS_CHECK
+    const char *dbg_lo[DBG_RANGES], *dbg_hi[DBG_RANGES];  // checking build: the address ranges this launch may touch
+    unsigned long long *dbg_count;                        // DEVICE counter of refused accesses
+    int dbg_n;
+#endif
     unsigned short cls_end[LAUNCH_MODELS][CLS_COUNT];  // per model: end of each class, relative to its slice
     LensK table[LAUNCH_RECORDS];
 };
@@ -60,6 +66,11 @@ struct EvalJob {
     cudaStream_t aux = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     double *stats_scratch = nullptr;  // stats + two chains: DEVICE, 18 planes (mean, m2 of the odd-model chain)
+#ifdef LH_BOUNDS_CHECK
+    const char *dbg_lo[DBG_RANGES], *dbg_hi[DBG_RANGES];
+    unsigned long long *dbg_count = nullptr;
+    int dbg_n = 0;
+#endif
 };
 
 // Enqueues every launch of the job on `stream`; adds the number of kernels launched to *launches.
