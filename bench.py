@@ -370,21 +370,25 @@ def run_ours(args):
     peer, peer_ptrs, owner_map = None, {}, None
     if scaling == "strong" and world > 1 and args.assemble in ("auto", "peer"):
         ok, err = 1, ""
-        try:
-            if rank == 0:
+        handles = [None]
+        if rank == 0:
+            try:
                 owner_map = {n: torch.empty((g.ny, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs}
                 handles = [{n: lh.lh_ipc_export(t) for n, t in owner_map.items()}]
-            else:
-                handles = [None]
-            dist.broadcast_object_list(handles, src=0)
-            if rank == 0:
-                peer = {n: owner_map[n][j0:j0 + nrows] for n in cfg.outputs}
-            else:
+            except Exception as e:  # e.g. an allocator whose memory cannot be exported
+                ok, err, handles = 0, repr(e), [None]
+        dist.broadcast_object_list(handles, src=0)  # every rank takes part, whatever happened on rank 0
+        if handles[0] is None:
+            ok = 0
+        elif rank == 0:
+            peer = {n: owner_map[n][j0:j0 + nrows] for n in cfg.outputs}
+        else:
+            try:
                 for n in cfg.outputs:
                     peer_ptrs[n] = lh.lh_ipc_open(*handles[0][n])
                 peer = {n: peer_ptrs[n] + j0 * g.nx * 8 for n in cfg.outputs}  # address of this rank's first row
-        except Exception as e:  # no IPC / no peer access on this machine: fall back to the gather
-            ok, err = 0, repr(e)
+            except Exception as e:  # no peer access between the two devices: fall back to the gather
+                ok, err = 0, repr(e)
         t = torch.tensor([float(ok)], dtype=torch.float64, device=red_dev)
         dist.all_reduce(t, op=dist.ReduceOp.MIN)
         if float(t.item()) < 1.0:
@@ -417,7 +421,12 @@ def run_ours(args):
             step()
             b.record(stream)
         barrier()
-    launches = lh.lh_launch_count() - launches0
+    launches = lh.lh_launch_count() - launches0  # this rank's
+    launches_all = launches
+    if world > 1:
+        t = torch.tensor([float(launches)], dtype=torch.float64, device=red_dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        launches_all = int(t.item())
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = reduce_max(sum(step_ms))  # MAX over ranks of the device time of the K steps
     ms_per_step = total_ms / args.steps
@@ -586,7 +595,9 @@ def run_ours(args):
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, **{k: v for k, v in stats_of(step_ms).items() if k != "n"},
             "higher_is_better": True, "scaling": scaling if world > 1 else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args, world, scaling),
-            "clocks": clk.summary(), "gpu_launches": int(launches), "roofline": roofline}
+            "clocks": clk.summary(), "gpu_launches": int(launches_all), "roofline": roofline}
+    if world > 1:
+        line["gpu_launches_rank0"] = int(launches)
     if not args.stats:
         sub = cfg if scaling != "strong" else None
         if sub is not None:

@@ -617,7 +617,8 @@ def test_bench_strong_scaling_arm_two_ranks_over_gloo(assemble):
     lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
     assert len(lines) == 1, r.stdout[-2000:]
     d = json.loads(lines[0])
-    assert d["n_gpus"] == 2 and d["scaling"] == "strong" and d["gpu_launches"] == 3  # rank 0: one launch per step
+    assert d["n_gpus"] == 2 and d["scaling"] == "strong"
+    assert d["gpu_launches"] == 6 and d["gpu_launches_rank0"] == 3  # one launch per rank and step
     assert d["assemble"]["mode"] == assemble
     assert d["assemble"]["bitwise_check"] is True and d["assemble"]["bytes"] == 2 * 1024 * 1024 * 8
     assert d["parity_last_step"]["ok"] and d["e2e"]["same_bits_as_device_planes"] is True
