@@ -41,11 +41,18 @@ namespace lh {
 #ifndef LH_MINB_HESS
 #define LH_MINB_HESS 5  // Hessian-only variant
 #endif
-constexpr int PX = LH_PX;
-constexpr int TILE_W = 32 * PX;    // one warp spans 32*PX pixels of a row
+#ifndef LH_PX_GRAD
+#define LH_PX_GRAD 8  // gradient-only variant: its lens loop is short enough for 8 pixels in 168 registers
+#endif
+// Pixels per thread of a kernel variant.  More pixels amortise the per-lens overhead (20 uniform loads + loop control)
+// over more evaluations: 79.1 instead of 81 instructions per gradient-only evaluation at 8.  The gradient + Hessian
+// variant stays at 4: at 8 it needs either 254 registers (8 warps per SM: latency shows, 87 ms) or, held to 168,
+// a schedule with exposed FP64 latency (96 ms) -- measured, DESIGN.md sec. 8b.
+template <bool GRAD, bool HESS>
+__host__ __device__ constexpr int px_of() { return (GRAD && !HESS) ? LH_PX_GRAD : LH_PX; }
 constexpr int TILE_H = LH_WARPS;
 constexpr int THREADS = 32 * TILE_H;
-static_assert(PX % 2 == 0, "PX must be even (double2 stores)");
+static_assert(LH_PX % 2 == 0 && LH_PX_GRAD % 2 == 0, "pixels per thread must be even (double2 stores)");
 
 struct Acc {
     double ax, ay, S, Dl, a12;
@@ -262,6 +269,8 @@ __global__ void __launch_bounds__(THREADS, EXTREME ? 1 : min_blocks<GRAD, HESS>(
         for (int t = threadIdx.x; t < (int)(sizeof(SmemTables) / sizeof(double2)); t += THREADS) dst[t] = LH_LDG(src + t);
     }
 
+    constexpr int PX = px_of<GRAD, HESS>();
+    constexpr int TILE_W = 32 * PX;  // one warp spans 32*PX pixels of a row
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tx = blockIdx.x % P.tiles_x, ty = blockIdx.x / P.tiles_x;
     const int i0 = tx * TILE_W + lane * PX;
@@ -462,12 +471,13 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     Q.px = J.px; Q.py = J.py;
     Q.carry = J.carry;
     Q.math = J.math;
-    Q.tiles_x = (J.nx + TILE_W - 1) / TILE_W;
-    const long long tiles = (long long)Q.tiles_x * ((J.ny + TILE_H - 1) / TILE_H);
-    if (tiles > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     const bool grad = J.out[0] || J.out[1];
     bool hess = false;
     for (int k = 2; k < 9; ++k) hess = hess || J.out[k];
+    const int tile_w = 32 * ((grad && !hess) ? px_of<true, false>() : px_of<true, true>());  // the variant's tile width
+    Q.tiles_x = (J.nx + tile_w - 1) / tile_w;
+    const long long tiles = (long long)Q.tiles_x * ((J.ny + TILE_H - 1) / TILE_H);
+    if (tiles > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
 
     cudaStream_t cur = stream;  // stream the next launch goes to (`stream`, or J.aux for every other chunked model)
     auto go = [&](int nm, bool extreme) -> cudaError_t {
