@@ -42,10 +42,10 @@ UNIT = "evals/s"
 
 # Executed FP64 thread-instructions per (pixel, lens) dPIE evaluation of each kernel variant, (DFMA, DMUL, DADD), read
 # from the SASS of the lens loop of the built library: tests/test_sass_cpu.py RECOUNTS them with cuobjdump and fails
-# when these constants and the kernel drift apart (the loop holds 4 evaluations, 8 in the gradient-only variant, whose
-# per-row subexpressions are therefore shared by 8).  flop = 2 DFMA + DMUL + DADD.
+# when these constants and the kernel drift apart (the loop holds 4 evaluations, 8 in the gradient-only and the Hessian-only
+# variants, whose per-row subexpressions are therefore shared by 8).  flop = 2 DFMA + DMUL + DADD.
 # This is what the hardware did -- `roofline.achieved` never claims more.  DESIGN.md sec. 7.
-FP64_OPS_PER_EVAL = {"grad+hess": (40.0, 28.75, 10.25), "grad": (30.0, 16.25, 9.125), "hess": (22.0, 16.75, 6.25)}
+FP64_OPS_PER_EVAL = {"grad+hess": (40.0, 28.75, 10.25), "grad": (30.0, 16.25, 9.125), "hess": (22.0, 16.375, 6.125)}
 FP64_INSTR_PER_EVAL = {k: sum(v) for k, v in FP64_OPS_PER_EVAL.items()}
 FLOPS_PER_EVAL = {k: 2 * v[0] + v[1] + v[2] for k, v in FP64_OPS_PER_EVAL.items()}
 # SURVEY.md sec. 8(d) canonical count for the cheapest exact formulation it knew (context: this kernel's
@@ -269,7 +269,7 @@ def sampled_parity(torch, cfg, out, model=0, n=1000, seed=2026):
 # tests/test_sass_cpu.py) -- only used for the FP64 issue fraction of the mixed config 2
 FP64_INSTR_PER_EVAL_CLASS = {"grad+hess": {"dpie": 79.0, "nsie": 57.0, "sis": 17.75},
                              "grad": {"dpie": 55.375, "nsie": 41.375, "sis": 10.25},
-                             "hess": {"dpie": 45.0, "nsie": 30.0, "sis": 15.75}}
+                             "hess": {"dpie": 44.5, "nsie": 29.5, "sis": 15.375}}
 
 
 def fp64_instr_of(cfg, mode):

@@ -49,7 +49,10 @@ namespace lh {
 // variant stays at 4: at 8 it needs either 254 registers (8 warps per SM: latency shows, 87 ms) or, held to 168,
 // a schedule with exposed FP64 latency (96 ms) -- measured, DESIGN.md sec. 8b.
 template <bool GRAD, bool HESS>
-__host__ __device__ constexpr int px_of() { return (GRAD && !HESS) ? LH_PX_GRAD : LH_PX; }
+#ifndef LH_PX_HESS
+#define LH_PX_HESS 8  // Hessian-only variant: no table look-ups, 8 pixels fit 168 registers without a spill
+#endif
+__host__ __device__ constexpr int px_of() { return (GRAD && !HESS) ? LH_PX_GRAD : ((HESS && !GRAD) ? LH_PX_HESS : LH_PX); }
 constexpr int TILE_H = LH_WARPS;
 constexpr int THREADS = 32 * TILE_H;
 static_assert(LH_PX % 2 == 0 && LH_PX_GRAD % 2 == 0, "pixels per thread must be even (double2 stores)");
@@ -474,7 +477,7 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     const bool grad = J.out[0] || J.out[1];
     bool hess = false;
     for (int k = 2; k < 9; ++k) hess = hess || J.out[k];
-    const int tile_w = 32 * ((grad && !hess) ? px_of<true, false>() : px_of<true, true>());  // the variant's tile width
+    const int tile_w = 32 * ((grad && !hess) ? px_of<true, false>() : ((hess && !grad) ? px_of<false, true>() : px_of<true, true>()));  // the variant's tile width
     Q.tiles_x = (J.nx + tile_w - 1) / tile_w;
     const long long tiles = (long long)Q.tiles_x * ((J.ny + TILE_H - 1) / TILE_H);
     if (tiles > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
