@@ -279,8 +279,9 @@ def fp64_instr_of(cfg, mode):
     return float(np.sum(t == li.DPIE) * k["dpie"] + np.sum(t == li.NSIE) * k["nsie"] + np.sum(t == li.SIS) * k["sis"])
 
 
-def config_block(torch, lh, stream, flush, which=(0, 1, 2, 4), steps=5):
-    """ms/step, evals/s and FP64 issue fraction of the other BASELINE configs (device-resident, CUDA events)."""
+def config_block(torch, lh, stream, flush, which=(0, 1, 2, 4), steps=5, oracle_too=True):
+    """ms/step, evals/s and FP64 issue fraction of the other BASELINE configs (device-resident, CUDA events), and the
+    single-thread oracle rate beside each (the whole map for cfg 0-1, a 64-row slab for cfg 2, 4)."""
     block = {}
     for idx in which:
         c = li.config(idx)
@@ -302,6 +303,9 @@ def config_block(torch, lh, stream, flush, which=(0, 1, 2, 4), steps=5):
             "traffic": NCU_TRAFFIC_BYTES.get(idx),
             "parity_last_step": sampled_parity(torch, c, out, model=c.nmodel - 1, n=300)}
         del out
+        if oracle_too:
+            one, _ = oracle_sample(c, 0.0, threads=1, min_rows=g.ny if idx <= 1 else 64)
+            block[f"cfg{idx}"]["oracle_single_thread"] = {k: one[k] for k in ("value", "unit", "cores", "sample")}
     return block
 
 
@@ -612,7 +616,7 @@ def run_ours(args):
     if e2e:
         line["e2e"] = e2e
     if world == 1 and not args.no_configs and args.config == 3 and not args.stats:
-        line["configs"] = config_block(torch, lh, stream, flush)
+        line["configs"] = config_block(torch, lh, stream, flush, oracle_too=not args.no_cpu_baseline)
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], _ = oracle_sample(cfg, args.cpu_seconds)
         one, _ = oracle_sample(cfg, 0.0, threads=1, min_rows=64 if cfg.evals > 2e9 else g.ny)

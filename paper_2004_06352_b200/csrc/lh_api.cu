@@ -2,11 +2,13 @@
 // staging of the packed table, launch.  No arithmetic of the method lives here.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
 #include <mutex>
+#include <thread>
 #include <new>
 #include <vector>
 
@@ -53,6 +55,9 @@ struct DeviceState {
     static const int PIECES = 8;  // pipeline depth of the *_host entry point (compute piece k+1 | copy piece k)
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_piece[PIECES] = {};
+    cudaEvent_t ev_copied[PIECES] = {};  // piece k has landed in the pinned ring (pageable host planes only)
+    char *h_ring = nullptr;              // pinned bounce ring of the *_host entry points: 2 slots
+    size_t ring_bytes = 0;
     double *d_sink = nullptr;
     char *d_chi = nullptr;  // scratch of lh_chi2 (deflection planes, constraint arrays, sources, images)
     size_t chi_bytes = 0;
@@ -626,6 +631,24 @@ namespace {
 
 // HOST output planes.  One map (nmodel == 1): rows [j0, j0 + nrows) of the grid into planes of nrows x nx doubles;
 // a batch: all rows of every model.
+// Host copy of one piece out of the pinned ring into the caller's pageable planes, on a few threads (one thread
+// moves 8-12 GB/s; the step would otherwise wait for it).
+void parallel_copy(char *dst, const char *src, size_t bytes) {
+    unsigned hw = std::thread::hardware_concurrency();
+    const int nt = (int)std::min<size_t>(hw ? (hw > 8 ? 8 : hw) : 1, bytes / (4u << 20) + 1);
+    if (nt <= 1) { std::memcpy(dst, src, bytes); return; }
+    std::vector<std::thread> th;
+    const size_t per = ((bytes / nt) + 4095) & ~size_t(4095);
+    for (int t = 1; t < nt; ++t) {
+        const size_t o = per * t;
+        if (o >= bytes) break;
+        const size_t n = bytes - o < per ? bytes - o : per;
+        th.emplace_back([=] { std::memcpy(dst + o, src + o, n); });
+    }
+    std::memcpy(dst, src, per < bytes ? per : bytes);
+    for (auto &t : th) t.join();
+}
+
 int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, int j0, int nrows, const lh_outputs *host_o) {
     ctx.err[0] = 0;
     int rc = check_common(lenses, nmodel, nlens, g);
@@ -669,7 +692,21 @@ int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, in
     // device-to-host copy of piece k runs on a second stream while piece k+1 is being computed.
     if (!DS().copy_stream) {
         CU(cudaStreamCreateWithFlags(&DS().copy_stream, cudaStreamNonBlocking));
-        for (int k = 0; k < DeviceState::PIECES; ++k) CU(cudaEventCreateWithFlags(&DS().ev_piece[k], cudaEventDisableTiming));
+        for (int k = 0; k < DeviceState::PIECES; ++k) {
+            CU(cudaEventCreateWithFlags(&DS().ev_piece[k], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&DS().ev_copied[k], cudaEventDisableTiming));
+        }
+    }
+    // Pageable host planes: a device-to-pageable cudaMemcpyAsync is staged by the driver at about 6 GB/s and would BE the
+    // step (cfg 3: 139 ms against 84 ms of computing).  Such planes are served through a pinned ring of two slots
+    // instead: piece k is copied device -> ring at link speed while piece k+1 computes, and host threads move it
+    // ring -> caller's planes meanwhile.  Pinned (or registered) planes are written directly.
+    bool pageable = false;
+    for (int k = 0; k < NPLANES; ++k) {
+        if (!hp[k]) continue;
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, hp[k]) != cudaSuccess) { cudaGetLastError(); pageable = true; }
+        else if (at.type == cudaMemoryTypeUnregistered) pageable = true;
     }
     const size_t npix = (size_t)g->nx * g->ny;
     const int units = nmodel == 1 ? nrows : nmodel;  // rows or models
@@ -681,6 +718,34 @@ int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, in
     const int pieces = want < 1 ? 1 : (want > DeviceState::PIECES ? DeviceState::PIECES : (int)want);
     int per = (units + pieces - 1) / pieces;
     if (nmodel == 1) per = (per + 7) & ~7;            // whole pixel tiles
+    const size_t piece_elems = nmodel == 1 ? (size_t)per * g->nx : (size_t)per * npix;  // per plane, at most
+    const size_t slot_bytes = piece_elems * sizeof(double) * nreq;
+    if (pageable && 2 * slot_bytes > DS().ring_bytes) {
+        if (DS().h_ring) {
+            CU(cudaStreamSynchronize(DS().copy_stream));
+            cudaFreeHost(DS().h_ring);
+            DS().h_ring = nullptr;
+            DS().ring_bytes = 0;
+        }
+        CU(cudaMallocHost(&DS().h_ring, 2 * slot_bytes));
+        DS().ring_bytes = 2 * slot_bytes;
+    }
+    // ring -> caller's planes for piece q (blocks until its device -> ring copies have landed)
+    struct Pending { size_t off, count; int slot; bool live; } pend = {0, 0, 0, false};
+    auto drain = [&](int q) -> int {
+        if (!pend.live) return LH_OK;
+        CU(cudaEventSynchronize(DS().ev_copied[q]));
+        int s = 0;
+        for (int k = 0; k < NPLANES; ++k) {
+            if (!hp[k]) continue;
+            parallel_copy(reinterpret_cast<char *>(hp[k] + pend.off),
+                          DS().h_ring + (size_t)pend.slot * slot_bytes + (size_t)s * piece_elems * sizeof(double),
+                          pend.count * sizeof(double));
+            ++s;
+        }
+        pend.live = false;
+        return LH_OK;
+    };
     int piece = 0;
     for (int u0 = 0; u0 < units; u0 += per, ++piece) {
         const int nu = units - u0 < per ? units - u0 : per;
@@ -698,9 +763,24 @@ int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, in
         }
         CU(cudaEventRecord(DS().ev_piece[piece], ctx.stream));
         CU(cudaStreamWaitEvent(DS().copy_stream, DS().ev_piece[piece], 0));
-        for (int k = 0; k < NPLANES; ++k)
-            if (hp[k]) CU(cudaMemcpyAsync(hp[k] + off, dp[k] + off, count * sizeof(double), cudaMemcpyDeviceToHost, DS().copy_stream));
+        if (!pageable) {
+            for (int k = 0; k < NPLANES; ++k)
+                if (hp[k]) CU(cudaMemcpyAsync(hp[k] + off, dp[k] + off, count * sizeof(double), cudaMemcpyDeviceToHost, DS().copy_stream));
+            continue;
+        }
+        // slot piece % 2 is free: the piece that used it last (piece - 2) was drained during the previous iteration
+        int s = 0;
+        for (int k = 0; k < NPLANES; ++k) {
+            if (!hp[k]) continue;
+            CU(cudaMemcpyAsync(DS().h_ring + (size_t)(piece & 1) * slot_bytes + (size_t)s * piece_elems * sizeof(double), dp[k] + off,
+                               count * sizeof(double), cudaMemcpyDeviceToHost, DS().copy_stream));
+            ++s;
+        }
+        CU(cudaEventRecord(DS().ev_copied[piece], DS().copy_stream));
+        if ((rc = drain(piece - 1))) return rc;  // the PREVIOUS piece, while this one computes and copies
+        pend = {off, count, piece & 1, true};
     }
+    if (pageable && (rc = drain(piece - 1))) return rc;
     CU(cudaStreamSynchronize(DS().copy_stream));
     CU(cudaStreamSynchronize(ctx.stream));
     return LH_OK;
