@@ -27,7 +27,13 @@
 namespace lh {
 
 #ifndef LH_PX
-#define LH_PX 4  // pixels per thread (adjacent in x -> double2 stores; per-lens uniform loads amortised over 4)
+#define LH_PX 4  // pixels per thread, gradient + Hessian variant (adjacent in x -> double2 stores)
+#endif
+#ifndef LH_PX_GRAD
+#define LH_PX_GRAD 8  // gradient-only variant: its lens loop is short enough for 8 pixels in 168 registers
+#endif
+#ifndef LH_PX_HESS
+#define LH_PX_HESS 8  // Hessian-only variant: no table look-ups, 8 pixels fit 168 registers without a spill
 #endif
 #ifndef LH_WARPS
 #define LH_WARPS 2  // warps per CTA, one grid row each
@@ -41,21 +47,16 @@ namespace lh {
 #ifndef LH_MINB_HESS
 #define LH_MINB_HESS 5  // Hessian-only variant
 #endif
-#ifndef LH_PX_GRAD
-#define LH_PX_GRAD 8  // gradient-only variant: its lens loop is short enough for 8 pixels in 168 registers
-#endif
-// Pixels per thread of a kernel variant.  More pixels amortise the per-lens overhead (20 uniform loads + loop control)
-// over more evaluations: 79.1 instead of 81 instructions per gradient-only evaluation at 8.  The gradient + Hessian
-// variant stays at 4: at 8 it needs either 254 registers (8 warps per SM: latency shows, 87 ms) or, held to 168,
-// a schedule with exposed FP64 latency (96 ms) -- measured, DESIGN.md sec. 8b.
+// Pixels per thread of a kernel variant.  More pixels amortise the per-lens overhead (the uniform loads of the record
+// and the loop control) over more evaluations: 79.1 instead of 81 instructions per gradient-only evaluation at 8,
+// 52.75 instead of 56 per Hessian-only one.  The gradient + Hessian variant stays at 4: at 8 it needs either 254
+// registers (8 warps per SM: the FP64 latency shows, 87 ms) or, held to 168, a schedule that exposes it even more
+// (96 ms) -- measured, DESIGN.md sec. 8b.
 template <bool GRAD, bool HESS>
-#ifndef LH_PX_HESS
-#define LH_PX_HESS 8  // Hessian-only variant: no table look-ups, 8 pixels fit 168 registers without a spill
-#endif
 __host__ __device__ constexpr int px_of() { return (GRAD && !HESS) ? LH_PX_GRAD : ((HESS && !GRAD) ? LH_PX_HESS : LH_PX); }
 constexpr int TILE_H = LH_WARPS;
 constexpr int THREADS = 32 * TILE_H;
-static_assert(LH_PX % 2 == 0 && LH_PX_GRAD % 2 == 0, "pixels per thread must be even (double2 stores)");
+static_assert(LH_PX % 2 == 0 && LH_PX_GRAD % 2 == 0 && LH_PX_HESS % 2 == 0, "pixels per thread must be even (double2 stores)");
 
 struct Acc {
     double ax, ay, S, Dl, a12;
