@@ -66,6 +66,8 @@ struct DeviceState {
     bool chi_busy = false;
     cudaStream_t aux_stream = nullptr;  // second launch chain of batches of chunked models (lh_kernels.cu)
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaStream_t piece_stream = nullptr;  // the odd pieces of the *_host entry points (one map): their launch tails overlap
+    cudaEvent_t ev_pfork = nullptr, ev_pjoin = nullptr;
 };
 
 struct Context {
@@ -180,6 +182,10 @@ struct EvalOpts {
     // >= 0: the models were validated and packed into ctx.h_table / ctx.h_ranges by pack_all() already and this job
     // evaluates `nmodel` of them starting at model `packed0` (`lenses` is then not read)
     int packed0 = -1;
+    // the caller has already made the carry buffer safe for this job and will record its end of use itself (the pieces
+    // of eval_host alternate between two streams and touch disjoint rows of one carry buffer)
+    bool carry_guard_by_caller = false;
+    cudaStream_t stream_override = nullptr;  // != nullptr: enqueue on this stream instead of the thread's
 };
 
 // a1 for a whole call: validate + pack nmodel x nlens lenses into ctx.h_table / ctx.h_ranges.  Nothing is enqueued.
@@ -238,7 +244,7 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
             return LH_EINVAL;
     }
 
-    cudaStream_t s = ctx.stream;
+    cudaStream_t s = opt.stream_override ? opt.stream_override : ctx.stream;
     const size_t carry_one =
         (nlens > lh::LAUNCH_RECORDS || nshared > 0) ? (size_t)5 * g->nx * g->ny * sizeof(double) : 0;
     // batches of chunked models run as two interleaved launch chains, each with a carry buffer of its own
@@ -251,7 +257,7 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
         CU(cudaEventCreateWithFlags(&DS().ev_fork, cudaEventDisableTiming));
         CU(cudaEventCreateWithFlags(&DS().ev_join, cudaEventDisableTiming));
     }
-    {
+    if (!opt.carry_guard_by_caller) {
         int rc = ensure_carry(carry_need, s);
         if (rc) return rc;
     }
@@ -309,7 +315,7 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     ++J.dbg_n;
 #endif
     CU(lh::launch_eval(J, s, &ctx.launches));
-    if (carry_need) {
+    if (carry_need && !opt.carry_guard_by_caller) {
         CU(cudaEventRecord(DS().ev_done, s));
         DS().busy = true;
         DS().last_stream = s;
@@ -730,6 +736,22 @@ int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, in
         CU(cudaMallocHost(&DS().h_ring, 2 * slot_bytes));
         DS().ring_bytes = 2 * slot_bytes;
     }
+    // One map: the pieces are independent (disjoint rows of the planes AND of the carry buffer), so the odd ones go to
+    // a second stream and the part-filled last wave of one piece's launches is filled by the next piece's CTAs.
+    // (Not with pageable planes: there the host drains piece k-1 before it enqueues piece k+1, and two pieces sharing
+    // the GPU would make it wait longer for k-1 and starve the queue -- measured 96.8 ms against 91.6.)
+    const bool two_streams = nmodel == 1 && pieces > 1 && !pageable;
+    cudaStream_t user_stream = ctx.stream;
+    if (two_streams) {
+        if (!DS().piece_stream) {
+            CU(cudaStreamCreateWithFlags(&DS().piece_stream, cudaStreamNonBlocking));
+            CU(cudaEventCreateWithFlags(&DS().ev_pfork, cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&DS().ev_pjoin, cudaEventDisableTiming));
+        }
+        if (nlens > lh::LAUNCH_RECORDS && (rc = ensure_carry((size_t)5 * g->nx * nrows * sizeof(double), user_stream))) return rc;
+        CU(cudaEventRecord(DS().ev_pfork, user_stream));
+        CU(cudaStreamWaitEvent(DS().piece_stream, DS().ev_pfork, 0));
+    }
     // ring -> caller's planes for piece q (blocks until its device -> ring copies have landed)
     struct Pending { size_t off, count; int slot; bool live; } pend = {0, 0, 0, false};
     auto drain = [&](int q) -> int {
@@ -756,12 +778,18 @@ int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, in
         EvalOpts opt;
         if (nmodel == 1) { opt.j0 = j0 + u0; opt.nrows = nu; opt.buf_row0 = u0; opt.packed0 = 0; }
         else opt.packed0 = u0;
+        cudaStream_t pstream = user_stream;
+        if (two_streams) {
+            pstream = (piece & 1) ? DS().piece_stream : user_stream;
+            opt.stream_override = pstream;
+            opt.carry_guard_by_caller = true;
+        }
         rc = eval_device(lenses, nmodel == 1 ? 1 : nu, nlens, nmodel == 1 ? &slab : g, sub, opt);
         if (rc) {  // only a CUDA failure can get here: the lens lists were validated above
             cudaStreamSynchronize(DS().copy_stream);
             return rc;
         }
-        CU(cudaEventRecord(DS().ev_piece[piece], ctx.stream));
+        CU(cudaEventRecord(DS().ev_piece[piece], pstream));
         CU(cudaStreamWaitEvent(DS().copy_stream, DS().ev_piece[piece], 0));
         if (!pageable) {
             for (int k = 0; k < NPLANES; ++k)
@@ -781,6 +809,15 @@ int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, in
         pend = {off, count, piece & 1, true};
     }
     if (pageable && (rc = drain(piece - 1))) return rc;
+    if (two_streams) {  // join, and hand the carry buffer back to the ordinary one-stream protocol
+        CU(cudaEventRecord(DS().ev_pjoin, DS().piece_stream));
+        CU(cudaStreamWaitEvent(user_stream, DS().ev_pjoin, 0));
+        if (nlens > lh::LAUNCH_RECORDS) {
+            CU(cudaEventRecord(DS().ev_done, user_stream));
+            DS().busy = true;
+            DS().last_stream = user_stream;
+        }
+    }
     CU(cudaStreamSynchronize(DS().copy_stream));
     CU(cudaStreamSynchronize(ctx.stream));
     return LH_OK;
