@@ -58,7 +58,7 @@ FP64_LANES_PER_S = 148 * 64 * 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the timed kernel, from one `ncu --set full` capture per
 # config (profiles/r02_all_configs_ncu.md, profiles/r02_cfg3_ncu.md: a middle lens chunk where the model is chunked;
 # launches whose output fits the 126 MB L2 show almost no DRAM traffic inside the launch -- write-back caching)
-NCU_TRAFFIC_BYTES = {0: 1.05e5, 1: 1.01e5, 2: 1.482e8, 3: 1.28996e9, 4: 1.688e7}
+NCU_TRAFFIC_BYTES = {0: 1.04e5, 1: 1.02e5, 2: 5.44e7, 3: 6.191e8, 4: 1.688e7}
 
 
 def parse():

@@ -252,7 +252,11 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     const bool two_chains = nlens > lh::LAUNCH_RECORDS && nmodel > 1 && nshared == 0;
     const size_t stats_scratch = (two_chains && dev_m2) ? (size_t)18 * g->nx * g->ny * sizeof(double) : 0;
     const size_t carry_need = carry_one * (two_chains ? 2 : 1) + stats_scratch;
-    if (two_chains && !DS().aux_stream) {
+    // one chunked model on a grid: its two row halves run as two chains (lh_kernels.cu); not for the pieces of eval_host,
+    // which are two chains themselves
+    const bool row_halves = nlens > lh::LAUNCH_RECORDS && nmodel == 1 && !dev_m2 && nshared == 0 && !opt.px &&
+                            !opt.carry_guard_by_caller;
+    if ((two_chains || row_halves) && !DS().aux_stream) {
         CU(cudaStreamCreateWithFlags(&DS().aux_stream, cudaStreamNonBlocking));
         CU(cudaEventCreateWithFlags(&DS().ev_fork, cudaEventDisableTiming));
         CU(cudaEventCreateWithFlags(&DS().ev_join, cudaEventDisableTiming));
@@ -288,6 +292,11 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     // carry is laid out like the planes it serves (g->ny rows of g->nx): a piece that starts at row buf_row0 of
     // those planes uses the same rows of the carry buffer
     J.carry = DS().d_carry ? DS().d_carry + (size_t)opt.buf_row0 * g->nx : nullptr;
+    if (row_halves) {
+        J.aux = DS().aux_stream;
+        J.ev_fork = DS().ev_fork;
+        J.ev_join = DS().ev_join;
+    }
     if (two_chains) {
         J.carry2 = DS().d_carry + carry_one / sizeof(double);
         J.aux = DS().aux_stream;

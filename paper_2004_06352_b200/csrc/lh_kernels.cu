@@ -480,7 +480,7 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     for (int k = 2; k < 9; ++k) hess = hess || J.out[k];
     const int tile_w = 32 * ((grad && !hess) ? px_of<true, false>() : ((hess && !grad) ? px_of<false, true>() : px_of<true, true>()));  // the variant's tile width
     Q.tiles_x = (J.nx + tile_w - 1) / tile_w;
-    const long long tiles = (long long)Q.tiles_x * ((J.ny + TILE_H - 1) / TILE_H);
+    long long tiles = (long long)Q.tiles_x * ((J.ny + TILE_H - 1) / TILE_H);  // of the launch being prepared
     if (tiles > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
 
     cudaStream_t cur = stream;  // stream the next launch goes to (`stream`, or J.aux for every other chunked model)
@@ -554,8 +554,11 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     // (cfg 4: 4096 CTAs over 888 resident slots = 4.6 waves per launch).  Statistics mode folds the models in order
     // and stays on one stream.
     const bool two = J.aux != nullptr && J.carry2 != nullptr && J.nmodel > 1 && (!J.stats || J.stats_scratch != nullptr);
+    // ONE chunked model on a large grid: the launches of its chain each end in a part-filled wave, too.  Rows are
+    // independent, so the upper and the lower half of the rows run as two chains (same carry buffer, disjoint rows).
+    const bool halves = J.aux != nullptr && J.nmodel == 1 && !J.stats && !shared && !J.px && tiles >= 4 * 888 && J.ny >= 4 * TILE_H;
     cudaError_t e = cudaSuccess;
-    if (two) {
+    if (two || halves) {
         if ((e = cudaEventRecord(J.ev_fork, stream)) != cudaSuccess) return e;
         if ((e = cudaStreamWaitEvent(J.aux, J.ev_fork, 0)) != cudaSuccess) return e;
     }
@@ -565,6 +568,23 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     for (int k = 0; k < 9; ++k) {
         out1[k] = (J.stats && two && J.out[k]) ? J.stats_scratch + (size_t)k * J.plane : nullptr;
         m2_1[k] = (J.stats && two && J.m2[k]) ? J.stats_scratch + (size_t)(9 + k) * J.plane : nullptr;
+    }
+    if (halves) {
+        const int h = (J.ny / 2 + TILE_H - 1) / TILE_H * TILE_H;  // rows of the first half: whole tiles
+        for (int part = 0; part < 2 && e == cudaSuccess; ++part) {
+            const int r0 = part ? h : 0, rows = part ? J.ny - h : h;
+            cur = part ? J.aux : stream;
+            Q.ny = rows;
+            Q.j0 = J.j0 + r0;
+            Q.carry = J.carry + (size_t)r0 * J.nx;
+            for (int q = 0; q < 9; ++q) Q.out[q] = J.out[q] ? J.out[q] + (size_t)r0 * J.nx : nullptr;
+            tiles = (long long)Q.tiles_x * ((rows + TILE_H - 1) / TILE_H);
+            e = chunks(J.table, J.ranges[0], n, 0, true, true, 0);
+        }
+        cur = stream;
+        cudaError_t e2 = cudaEventRecord(J.ev_join, J.aux);
+        if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(stream, J.ev_join, 0);
+        return e == cudaSuccess ? e2 : e;
     }
     for (int m = 0; m < J.nmodel && e == cudaSuccess; ++m) {
         const bool odd = two && (m & 1);
