@@ -80,6 +80,17 @@ def chunked():
     return w
 
 
+def row_halves():
+    # one chunked model on a grid large enough for the two-chain split of its rows (lh_kernels.cu `halves`): ragged
+    # width, odd height, so that the half boundary and the last tile row are both exercised
+    g = li.Grid(x0=-90.0, y0=-91.0, dx=0.18, nx=1000, ny=1023)
+    names = ("ax", "kappa", "mu")
+    o = planes(names, (g.ny, g.nx))
+    allow(*o.values())
+    lh.lh_grid_eval(c3.lenses[:161], g, **o)
+    return max(check_planes(host(o), ref(c3.lenses[:161], g, names), "row halves").values())
+
+
 def slabs():
     c = li.config(2, scale=16)
     g = li.Grid(x0=c.grid.x0 + 0.1, y0=c.grid.y0 + 0.3, dx=c.grid.dx * 1.1, nx=c.grid.nx, ny=c.grid.ny)
@@ -157,6 +168,7 @@ def points():
 
 
 for name, fn in (("ragged grids, all planes", ragged), ("lens chunks through the carry buffer", chunked),
+                 ("one chunked model, row halves on two chains", row_halves),
                  ("row slabs of a chunked model, device and host planes", slabs),
                  ("batches: shared launches, two launch chains, host entry", batches),
                  ("statistics (two chains + merge) and shared-lens batch", stats_and_shared), ("arbitrary points", points)):
