@@ -124,6 +124,41 @@ int lh_grid_eval(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_ou
  * bit-identical to the same rows of lh_grid_eval.  0 <= j0, nrows >= 1, j0 + nrows <= ny. */
 int lh_grid_eval_rows(const lh_lens *lenses, int nlens, const lh_grid *g, int j0, int nrows, const lh_outputs *o);
 
+/* lh_grid_eval_rows for callers that must not allocate device memory.
+ *
+ * Who needs it.  The other entry points call cudaMalloc the first time they need their reduction tables and, for a
+ * lens list longer than one launch carries (160 lenses), the `carry` planes that hand the partial sums of a pixel
+ * from one launch to the next.  That is not acceptable to a program whose device memory is owned by someone else
+ * (a framework's caching allocator or a scheduler that has taken the whole GPU: the library's cudaMalloc fails or
+ * upsets the accounting), to a loop that must never stall (cudaMalloc / cudaFree synchronise the device), or where
+ * the rule is "reserve everything at start-up".  This call makes NO cudaMalloc, cudaFree, stream, event or other
+ * allocating CUDA call, and packs the lenses into a fixed host table: both buffers are `static __device__` arrays
+ * inside liblh.so, reserved by the CUDA loader on every GPU that loads the library and held until the process ends.
+ *
+ * Limits (the price of a fixed reservation): nx*nrows <= LH_NOALLOC_MAX_PIXELS and nlens <= LH_NOALLOC_MAX_LENSES;
+ * beyond either the call returns LH_EINVAL, says so in lh_last_error() and touches nothing.  A larger grid is
+ * covered by several calls, one row slab each (slabs are bit-identical to the same rows of lh_grid_eval).
+ * The reservation is 5 * LH_NOALLOC_MAX_PIXELS * 8 bytes = 40 MiB per GPU, plus 32 KB of tables.
+ *
+ * Arguments, layout, stream and result exactly as lh_grid_eval_rows: planes of nrows*nx doubles, row j0 first,
+ * DEVICE pointers owned by the caller; enqueued on the lh_set_stream() stream as ONE launch chain (no second
+ * stream), returns without synchronising.
+ *
+ * First call on each device: it looks up the device address of the two arrays (cudaGetSymbolAddress) and uploads
+ * the tables with a synchronous cudaMemcpy.  Make that call once per device during set-up, with that device
+ * current, and before any stream capture begins; later calls only pack and launch.
+ *
+ * One buffer for everybody.  Every call on a device uses the same scratch and leaves its last contents there.
+ * Nothing needs clearing: the first launch of a chain starts its sums at zero without reading the scratch, and
+ * every later launch reads only what the launch before it wrote for the same pixel.  For the same reason two calls
+ * whose kernels can OVERLAP on the GPU (different streams, or different host threads on different streams) race on
+ * it and produce garbage: keep the calls of one device on one stream, or order them with events.  Host-side the
+ * call is serialised by a mutex, so calling from several threads is safe as long as the streams are ordered.
+ * Not available in the checking build (liblh_check.so): LH_EINVAL there. */
+#define LH_NOALLOC_MAX_PIXELS (1 << 20)
+#define LH_NOALLOC_MAX_LENSES 4096
+int lh_grid_eval_noalloc(const lh_lens *lenses, int nlens, const lh_grid *g, int j0, int nrows, const lh_outputs *o);
+
 /* The same superposition at ARBITRARY points instead of a grid: xs, ys DEVICE [npoints]; every requested plane of
  * `o` holds npoints doubles.  (Stage 2 of the paper's chi^2 pipeline unlenses the observed images, which are not
  * on the grid: PAPER.md:76 Fig. 3, :192.)  Same kernels, same arithmetic; errors as lh_grid_gradient. */

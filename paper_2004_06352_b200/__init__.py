@@ -7,7 +7,7 @@ missing -- there is no CPU fallback (and it never imports `oracle`).
 
 Names mirror the C ABI one to one:
     lh_grid_gradient, lh_grid_hessian, lh_lens_maps, lh_grid_gradient_batch,
-    lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_grid_eval_rows_host, lh_grid_stats_batch, lh_pack_model, lh_set_stream,
+    lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_grid_eval_rows_host, lh_grid_eval_noalloc, lh_grid_stats_batch, lh_pack_model, lh_set_stream,
     lh_ipc_export, lh_ipc_open, lh_ipc_close, lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_math_host_eval,
     lh_version
 Outputs may be torch CUDA tensors (float64, contiguous), anything with a
@@ -79,6 +79,8 @@ def _load():
         L.lh_points_eval.restype = ci
         L.lh_grid_eval_rows.argtypes = [vp, ci, gp, ci, ci, op]
         L.lh_grid_eval_rows.restype = ci
+        L.lh_grid_eval_noalloc.argtypes = [vp, ci, gp, ci, ci, op]
+        L.lh_grid_eval_noalloc.restype = ci
         L.lh_grid_eval_batch_shared.argtypes = [vp, ci, vp, ci, ci, gp, op]
         L.lh_grid_eval_batch_shared.restype = ci
         L.lh_source_plane.argtypes = [dp, dp, gp, dp, dp]
@@ -223,6 +225,20 @@ def lh_grid_eval_rows(lenses, grid, j0: int, nrows: int, **planes):
     a, p, n = _lenses_ptr(lenses)
     o = _outputs(planes, _dev_ptr, int(nrows) * int(grid.nx))
     _check(_load().lh_grid_eval_rows(p, n, C.byref(_grid(grid)), int(j0), int(nrows), C.byref(o)))
+
+
+LH_NOALLOC_MAX_PIXELS, LH_NOALLOC_MAX_LENSES = 1 << 20, 4096
+
+
+def lh_grid_eval_noalloc(lenses, grid, j0: int, nrows: int, **planes):
+    """lh_grid_eval_rows for programs that must not let a library allocate device memory (a caching allocator owns
+    the GPU, a loop that may not stall on cudaMalloc, "reserve everything at start-up" rules): the scratch is a fixed
+    40 MiB array inside liblh.so.  At most LH_NOALLOC_MAX_PIXELS pixels per call and LH_NOALLOC_MAX_LENSES lenses,
+    else LhError(LH_EINVAL).  Make the first call on each device during set-up; keep all calls of a device on one
+    stream (they share the scratch).  Planes of shape [nrows, nx]; see include/lh.h."""
+    a, p, n = _lenses_ptr(lenses)
+    o = _outputs(planes, _dev_ptr, int(nrows) * int(grid.nx))
+    _check(_load().lh_grid_eval_noalloc(p, n, C.byref(_grid(grid)), int(j0), int(nrows), C.byref(o)))
 
 
 def lh_grid_eval_batch(lenses, nmodel, nlens, grid, **planes):

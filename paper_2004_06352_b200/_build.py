@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblh.so")
-SOURCES = ["lh_api.cu", "lh_kernels.cu", "lh_delens.cu", "lh_pack.cpp"]
+SOURCES = ["lh_api.cu", "lh_kernels.cu", "lh_delens.cu", "lh_noalloc.cu", "lh_pack.cpp"]
 HEADERS = ["lh_kernels.h", "lh_pack.h", "lh_math.cuh", os.path.join("..", "..", "include", "lh.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

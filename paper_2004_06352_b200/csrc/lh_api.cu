@@ -359,6 +359,15 @@ int eval_checked(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g,
 
 }  // namespace
 
+// What an entry point that lives in another file (lh_noalloc.cu) needs of this host thread's state: the stream of
+// lh_set_stream, the text behind lh_last_error and the counter behind lh_launch_count.
+namespace lh {
+cudaStream_t api_stream() { return ctx.stream; }
+int api_fail(int code, const char *msg) { return fail(code, "%s", msg); }
+void api_clear_error() { ctx.err[0] = 0; }
+long long *api_launch_counter() { return &ctx.launches; }
+}  // namespace lh
+
 extern "C" {
 
 int lh_grid_eval(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_outputs *o) {
