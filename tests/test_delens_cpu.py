@@ -111,6 +111,24 @@ def test_closed_triangle_rule_on_shared_edges_and_vertices():
     assert tri((np.nextafter(2.0, 3.0), 2.0)) == [] and tri((-2.0, np.nextafter(-1.0, -2.0))) == []
 
 
+def test_bounding_box_clause_decides_where_the_rounded_barycentric_test_cannot():
+    """R22's box clause, seen on its own.  No lens, coarse grid x in {-3, 1, 5}: the source
+    (1 + 1 ulp, 0) lies in cell 1 and, by the plain definition of a closed triangle, NOT in triangle 0 of cell 0,
+    whose vertices all have x <= 1.  In floating point S - A = 4 + 2.2e-16 rounds to B - A = 4 exactly, so the
+    barycentric test alone gives u = 1, v = 0 and accepts it: without the box there are two images (triangles 0
+    and 2), with it one (triangle 2).  (On the finer grid of the test above S - A is exactly representable and u > 1
+    rejects the point either way -- that case does not see the clause; this one does.)  Mirrored on a y edge."""
+    one_up = np.nextafter(1.0, 2.0)
+    z = np.zeros((2, 3))
+    im, found = oracle.delens(z, z, -3.0, 0.0, 4.0, [[one_up, 0.0]])
+    assert found == 1 and [int(t) for t in im["triangle"]] == [2]
+    assert im["x"][0] == one_up and im["y"][0] == 0.0
+    z = np.zeros((3, 2))
+    im, found = oracle.delens(z, z, 0.0, -3.0, 4.0, [[0.0, one_up]])  # cells stacked in y; cell (0, 1) = triangles 2, 3
+    assert found == 1 and [int(t) for t in im["triangle"]] == [2]
+    assert im["x"][0] == 0.0 and im["y"][0] == one_up
+
+
 def test_sis_two_images_at_known_radii():
     """SIS, source at distance s < b0 from the centre: images on the source's ray at R = b0 + s and, on the
     opposite side, R = b0 - s (plus whatever the cells touching the singular centre produce, excluded here)."""

@@ -67,6 +67,21 @@ def test_delens_same_deflection_bit_exact(idx, scale, ns):
     assert np.all(a["_pad"] == 0)
 
 
+def test_bounding_box_clause_cases_agree_with_the_definition():
+    """The sources of tests/test_delens_cpu.py::test_bounding_box_clause_...: one ulp beyond a shared vertex, where
+    the rounded barycentric test alone would report a second image.  Expected values are the definition's (a closed
+    triangle lies in the box of its vertices), stated here as literals; the oracle must say the same."""
+    one_up = np.nextafter(1.0, 2.0)
+    for g, src, tri in ((li.Grid(x0=-3.0, y0=0.0, dx=4.0, nx=3, ny=2), [[one_up, 0.0]], 2),
+                        (li.Grid(x0=0.0, y0=-3.0, dx=4.0, nx=2, ny=3), [[0.0, one_up]], 2)):
+        z = np.zeros((g.ny, g.nx))
+        got, ngot = _gpu_delens(z, z, g, np.asarray(src))
+        want, nwant = oracle.delens(z, z, g.x0, g.y0, g.dx, src)
+        assert ngot == nwant == 1
+        assert int(got["triangle"][0]) == int(want["triangle"][0]) == tri
+        assert got["x"][0] == src[0][0] and got["y"][0] == src[0][1]
+
+
 def test_delens_whole_pipeline_own_deflection():
     """gradient on the GPU -> delens on the GPU, against gradient + delens in the oracle."""
     c = li.config(1, scale=4)
