@@ -419,6 +419,31 @@ def test_unrequested_planes_are_never_touched():
                 assert torch.isnan(out[n]).all()
 
 
+@pytest.mark.parametrize("which", ["cfg0", "chunked"])
+def test_every_subset_of_the_nine_planes(which):
+    """"every nullable-output combination of lh_grid_eval" -- all 511 non-empty subsets of the nine
+    planes.  The requested planes match the oracle, the others keep their NaN fill.  cfg 0 (10 lenses, one launch)
+    and a 500-lens mixed model (four launches through the carry buffer: the subset also decides which accumulators
+    are parked between launches)."""
+    c = li.config(0) if which == "cfg0" else li.config(2, scale=32)
+    g = c.grid
+    ref = ref_grid(c.lenses, g, li.ALL_PLANES)
+    buf = torch.empty((9, g.ny, g.nx), dtype=torch.float64, device="cuda")
+    worst = 0.0
+    for mask in range(1, 512):
+        req = [n for k, n in enumerate(li.ALL_PLANES) if mask >> k & 1]
+        buf.fill_(float("nan"))
+        lh.lh_grid_eval(c.lenses, g, **{n: buf[li.ALL_PLANES.index(n)] for n in req})
+        torch.cuda.synchronize()
+        host = buf.cpu().numpy()
+        for k, n in enumerate(li.ALL_PLANES):
+            if n not in req:
+                assert np.isnan(host[k]).all(), (req, n)
+        w = check_planes({n: host[li.ALL_PLANES.index(n)] for n in req}, ref, f"{which} subset {req}")
+        worst = max(worst, max(w.values()))
+    assert worst <= 1.0
+
+
 def test_guard_bands_not_overwritten():
     c = li.config(0)
     g = li.Grid(x0=-10.0, y0=-10.0, dx=0.3, nx=67, ny=5)
