@@ -266,9 +266,6 @@ int lh_set_stream(void *cuda_stream);
 /* Message for the last non-zero return on this host thread ("" if none). */
 const char *lh_last_error(void);
 
-/* Number of kernels this host thread has launched through the library so far. */
-long long lh_launch_count(void);
-
 /* Step a1 on its own (host only, no CUDA call): validate `n` lenses of one model and
  * write the per-lens constant table the kernels consume -- n records of
  * LH_PACK_DOUBLES doubles, sorted by evaluation class (stable inside a class) -- into
@@ -278,21 +275,6 @@ long long lh_launch_count(void);
 #define LH_PACK_DOUBLES 24
 #define LH_PACK_CLASSES 4
 int lh_pack_model(const lh_lens *lenses, int n, double *table, int32_t *class_begin);
-
-/* Diagnostic: runs a register-resident chain of dependent-free FP64 FMAs on every
- * SM for `iters` iterations and returns the achieved FP64 FLOP/s in *flops_per_s
- * (2 per FMA) and the kernel time in *seconds (CUDA events on the set stream;
- * synchronises).  Used by bench.py as the measured FP64 CUDA-core roofline. */
-int lh_fp64_peak_probe(int iters, double *flops_per_s, double *seconds);
-
-/* HOST evaluation of the kernel's own FP64 primitives (csrc/lh_math.cuh compiles for host and
- * device; on the host the 20-bit MUFU seeds are emulated by truncated exact quotients), so that
- * CPU-only tests can pin them against libm / arbitrary precision.  out[k] = fn(a[k], b[k]):
- *   fn 0  1/a            1  sqrt(a)        2  1/sqrt(a)
- *      3  atan(a/b), b > 0                 4  atanh(a/b), |a| < b, 1 - |a|/b > 2^-16
- *      5  1/a via the shared-seed pair (a, b)     6  1/a via the shared-seed quadruple (a, b, a+b, 2b)
- * No CUDA call is made.  LH_EINVAL for an unknown fn or a NULL pointer (b may be NULL for fn 0-2). */
-int lh_math_host_eval(int fn, const double *a, const double *b, size_t n, double *out);
 
 /* ---- several GPUs, one process each: writing a row slab straight into the owner's map ----
  * The output planes of lh_grid_eval_rows are plain device pointers, so a rank may hand it the address of ITS rows
@@ -316,6 +298,9 @@ int lh_ipc_close(void *dev_ptr);
 
 /* "lh <major>.<minor> sm_100a" */
 const char *lh_version(void);
+
+/* Diagnostics (launch counter, FP64 peak probe, host evaluation of the kernel's primitives, source hash, and the
+ * checking build's address-range calls) are declared in lh_diag.h: they serve bench.py and the tests, not the method. */
 
 #ifdef __cplusplus
 }

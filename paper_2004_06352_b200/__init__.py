@@ -9,7 +9,7 @@ Names mirror the C ABI one to one:
     lh_grid_gradient, lh_grid_hessian, lh_lens_maps, lh_grid_gradient_batch,
     lh_grid_eval, lh_grid_eval_batch, lh_grid_eval_host, lh_grid_eval_rows_host, lh_grid_eval_noalloc, lh_grid_stats_batch, lh_pack_model, lh_set_stream,
     lh_ipc_export, lh_ipc_open, lh_ipc_close, lh_last_error, lh_launch_count, lh_fp64_peak_probe, lh_math_host_eval,
-    lh_version
+    lh_version, lh_source_hash (the diagnostics are declared in include/lh_diag.h)
 Outputs may be torch CUDA tensors (float64, contiguous), anything with a
 `data_ptr()`, or raw integer device addresses.
 """
@@ -102,6 +102,7 @@ def _load():
         L.lh_math_host_eval.argtypes = [ci, vp, vp, C.c_size_t, vp]
         L.lh_math_host_eval.restype = ci
         L.lh_version.restype = C.c_char_p
+        L.lh_source_hash.restype = C.c_char_p
         for f in ("lh_grid_gradient", "lh_grid_hessian", "lh_lens_maps", "lh_grid_gradient_batch", "lh_grid_eval",
                   "lh_grid_eval_batch", "lh_grid_eval_host", "lh_set_stream", "lh_fp64_peak_probe"):
             getattr(L, f).restype = ci
@@ -404,3 +405,9 @@ def lh_math_host_eval(fn: int, a, b=None):
 
 def lh_version() -> str:
     return _load().lh_version().decode()
+
+
+def lh_source_hash() -> str:
+    """SHA-256 of the sources the loaded library was compiled from (include/lh_diag.h); compare with
+    _build.source_hash() to tell a stale prebuilt library from a current one."""
+    return _load().lh_source_hash().decode()

@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "../../include/lh.h"
+#include "../../include/lh_diag.h"
 #include "lh_kernels.h"
 
 namespace lh {
@@ -219,6 +220,14 @@ int ensure_carry(size_t need, cudaStream_t s) {
     return LH_OK;
 }
 
+// The second launch chain of chunked models (lh_kernels.cu): its stream and the fork / join events, made once per device.
+int ensure_aux_stream() {
+    if (!DS().aux_stream) CU(cudaStreamCreateWithFlags(&DS().aux_stream, cudaStreamNonBlocking));
+    if (!DS().ev_fork) CU(cudaEventCreateWithFlags(&DS().ev_fork, cudaEventDisableTiming));
+    if (!DS().ev_join) CU(cudaEventCreateWithFlags(&DS().ev_join, cudaEventDisableTiming));
+    return LH_OK;
+}
+
 int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, double *dev_out[NPLANES],
                 const EvalOpts &opt = EvalOpts()) {
     double **dev_m2 = opt.m2;
@@ -256,10 +265,9 @@ int eval_device(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, 
     // which are two chains themselves
     const bool row_halves = nlens > lh::LAUNCH_RECORDS && nmodel == 1 && !dev_m2 && nshared == 0 && !opt.px &&
                             !opt.carry_guard_by_caller;
-    if ((two_chains || row_halves) && !DS().aux_stream) {
-        CU(cudaStreamCreateWithFlags(&DS().aux_stream, cudaStreamNonBlocking));
-        CU(cudaEventCreateWithFlags(&DS().ev_fork, cudaEventDisableTiming));
-        CU(cudaEventCreateWithFlags(&DS().ev_join, cudaEventDisableTiming));
+    if (two_chains || row_halves) {
+        int rc = ensure_aux_stream();
+        if (rc) return rc;
     }
     if (!opt.carry_guard_by_caller) {
         int rc = ensure_carry(carry_need, s);
@@ -601,6 +609,7 @@ int lh_chi2(const lh_lens *lenses, int nlens, const lh_grid *g, const lh_constra
     if (nlens > lh::LAUNCH_RECORDS) {
         const size_t big = npix > (size_t)K ? npix : (size_t)K;
         if ((rc = ensure_carry((size_t)5 * big * sizeof(double), s))) return rc;
+        if ((rc = ensure_aux_stream())) return rc;  // stage 1 runs its row halves as two chains (eval_device)
     }
     int dev = 0, sms = 0;
     CU(cudaGetDevice(&dev));
@@ -661,16 +670,28 @@ void parallel_copy(char *dst, const char *src, size_t bytes) {
     unsigned hw = std::thread::hardware_concurrency();
     const int nt = (int)std::min<size_t>(hw ? (hw > 8 ? 8 : hw) : 1, bytes / (4u << 20) + 1);
     if (nt <= 1) { std::memcpy(dst, src, bytes); return; }
-    std::vector<std::thread> th;
+    // No exception may cross the C ABI (lh.h) and a joinable std::thread must never be destroyed: the helpers live in
+    // a fixed array (no allocation that could throw between two spawns), and a spawn that fails (EAGAIN under a pid
+    // limit) leaves its share, and every share after it, to the calling thread.
+    std::thread th[8];
+    int started = 0;
     const size_t per = ((bytes / nt) + 4095) & ~size_t(4095);
-    for (int t = 1; t < nt; ++t) {
+    size_t done_to = per < bytes ? per : bytes;  // the calling thread copies [0, per) and whatever no helper took
+    for (int t = 1; t < nt && t <= 8; ++t) {
         const size_t o = per * t;
         if (o >= bytes) break;
         const size_t n = bytes - o < per ? bytes - o : per;
-        th.emplace_back([=] { std::memcpy(dst + o, src + o, n); });
+        try {
+            th[started] = std::thread([=] { std::memcpy(dst + o, src + o, n); });
+        } catch (...) {
+            break;
+        }
+        ++started;
+        done_to = o + n;
     }
     std::memcpy(dst, src, per < bytes ? per : bytes);
-    for (auto &t : th) t.join();
+    if (done_to < bytes) std::memcpy(dst + done_to, src + done_to, bytes - done_to);
+    for (int t = 0; t < started; ++t) th[t].join();
 }
 
 int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, int j0, int nrows, const lh_outputs *host_o) {
@@ -786,6 +807,11 @@ int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, in
         pend.live = false;
         return LH_OK;
     };
+    // The pieces, as one unit that may stop early: whatever it returns, the epilogue below joins the streams, hands
+    // the carry buffer back and waits for everything that was enqueued (a failure on a later piece must not leave
+    // piece_stream unjoined or kernels running on a carry buffer the next call might free).
+    auto pipeline = [&]() -> int {
+    int rc = LH_OK;
     int piece = 0;
     for (int u0 = 0; u0 < units; u0 += per, ++piece) {
         const int nu = units - u0 < per ? units - u0 : per;
@@ -803,10 +829,7 @@ int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, in
             opt.carry_guard_by_caller = true;
         }
         rc = eval_device(lenses, nmodel == 1 ? 1 : nu, nlens, nmodel == 1 ? &slab : g, sub, opt);
-        if (rc) {  // only a CUDA failure can get here: the lens lists were validated above
-            cudaStreamSynchronize(DS().copy_stream);
-            return rc;
-        }
+        if (rc) return rc;  // only a CUDA failure can get here: the lens lists were validated above
         CU(cudaEventRecord(DS().ev_piece[piece], pstream));
         CU(cudaStreamWaitEvent(DS().copy_stream, DS().ev_piece[piece], 0));
         if (!pageable) {
@@ -827,18 +850,27 @@ int eval_host(const lh_lens *lenses, int nmodel, int nlens, const lh_grid *g, in
         pend = {off, count, piece & 1, true};
     }
     if (pageable && (rc = drain(piece - 1))) return rc;
+    return LH_OK;
+    };
+    rc = pipeline();
+    // epilogue, after success and failure alike; the FIRST error keeps its message
+    int rc2 = LH_OK;
+    auto keep = [&](cudaError_t e, const char *what) {
+        if (e != cudaSuccess && rc == LH_OK && rc2 == LH_OK) rc2 = fail(LH_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+    };
     if (two_streams) {  // join, and hand the carry buffer back to the ordinary one-stream protocol
-        CU(cudaEventRecord(DS().ev_pjoin, DS().piece_stream));
-        CU(cudaStreamWaitEvent(user_stream, DS().ev_pjoin, 0));
+        keep(cudaEventRecord(DS().ev_pjoin, DS().piece_stream), "cudaEventRecord(ev_pjoin)");
+        keep(cudaStreamWaitEvent(user_stream, DS().ev_pjoin, 0), "cudaStreamWaitEvent(ev_pjoin)");
         if (nlens > lh::LAUNCH_RECORDS) {
-            CU(cudaEventRecord(DS().ev_done, user_stream));
+            keep(cudaEventRecord(DS().ev_done, user_stream), "cudaEventRecord(ev_done)");
             DS().busy = true;
             DS().last_stream = user_stream;
         }
     }
-    CU(cudaStreamSynchronize(DS().copy_stream));
-    CU(cudaStreamSynchronize(ctx.stream));
-    return LH_OK;
+    keep(cudaStreamSynchronize(DS().copy_stream), "cudaStreamSynchronize(copy stream)");
+    keep(cudaStreamSynchronize(ctx.stream), "cudaStreamSynchronize");
+    pend.live = false;  // nothing is in flight any more: a ring slot with an undrained piece is simply abandoned
+    return rc ? rc : rc2;
 }
 
 }  // namespace
@@ -1012,5 +1044,10 @@ int lh_math_host_eval(int fn, const double *a, const double *b, size_t n, double
 }
 
 const char *lh_version(void) { return "lh 0.1 sm_100a"; }
+
+#ifndef LH_SOURCE_HASH
+#define LH_SOURCE_HASH "unknown"
+#endif
+const char *lh_source_hash(void) { return LH_SOURCE_HASH; }
 
 }  // extern "C"

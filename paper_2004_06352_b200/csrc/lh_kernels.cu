@@ -455,6 +455,26 @@ static cudaError_t launch_one(const LaunchParams &P, dim3 grid, cudaStream_t str
     return cudaGetLastError();
 }
 
+// CTAs of a variant that one device holds at once (occupancy x SM count): the size of a "wave" for the row-halves
+// decision below.  Asked of the runtime, per device and variant, once; the launch bounds (LH_MINB*) and the static
+// shared memory of the kernel are what it depends on.  0 if the query fails (the caller then keeps one chain).
+static long long resident_ctas(bool grad, bool hess) {
+    static int cache[64][3];  // 0 = not asked yet
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 0;
+    const int v = (grad && hess) ? 0 : (grad ? 1 : 2);
+    if (!cache[dev][v]) {
+        int per_sm = 0, sms = 0;
+        cudaError_t e = v == 0 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, superpose_kernel<true, true, false, false>, THREADS, 0)
+                      : v == 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, superpose_kernel<true, false, false, false>, THREADS, 0)
+                               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, superpose_kernel<false, true, false, false>, THREADS, 0);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) { cudaGetLastError(); return 0; }
+        cache[dev][v] = per_sm * sms > 0 ? per_sm * sms : -1;
+    }
+    return cache[dev][v] > 0 ? cache[dev][v] : 0;
+}
+
 // Host side of a6 and of the lens chunking: cut the packed tables into launches of at most
 // LAUNCH_RECORDS records.  Models with few lenses share a launch (blockIdx.y = model); a model
 // with more lenses than fit is evaluated by consecutive launches that hand the accumulators on
@@ -551,12 +571,14 @@ cudaError_t launch_eval(const EvalJob &J, cudaStream_t stream, long long *launch
     // one model at a time, balanced lens chunks.  The chunks of ONE model depend on each other through `carry`;
     // different models do not.  With a second stream and a second carry buffer the even and the odd models form two
     // independent chains, so the partial last wave of one chain's launch is filled by the other chain's CTAs
-    // (cfg 4: 4096 CTAs over 888 resident slots = 4.6 waves per launch).  Statistics mode folds the models in order
-    // and stays on one stream.
+    // (cfg 4: 4096 CTAs over 888 resident slots = 4.6 waves per launch).  Statistics mode uses the two chains as
+    // well when the caller gave it scratch planes for the odd-model chain (merge_stats_kernel joins the two).
     const bool two = J.aux != nullptr && J.carry2 != nullptr && J.nmodel > 1 && (!J.stats || J.stats_scratch != nullptr);
     // ONE chunked model on a large grid: the launches of its chain each end in a part-filled wave, too.  Rows are
     // independent, so the upper and the lower half of the rows run as two chains (same carry buffer, disjoint rows).
-    const bool halves = J.aux != nullptr && J.nmodel == 1 && !J.stats && !shared && !J.px && tiles >= 4 * 888 && J.ny >= 4 * TILE_H;
+    // Worth it from four waves of the variant's resident CTAs on (B200: 148 SMs x 5 or 6 CTAs = 740 / 888).
+    const long long wave = (J.aux != nullptr && J.nmodel == 1) ? resident_ctas(grad, hess) : 0;
+    const bool halves = J.aux != nullptr && J.nmodel == 1 && !J.stats && !shared && !J.px && wave > 0 && tiles >= 4 * wave && J.ny >= 4 * TILE_H;
     cudaError_t e = cudaSuccess;
     if (two || halves) {
         if ((e = cudaEventRecord(J.ev_fork, stream)) != cudaSuccess) return e;

@@ -22,6 +22,14 @@ import paper_2004_06352_b200 as lh  # noqa: E402
 from parity import check_planes, stats_violation  # noqa: E402
 
 lib = C.CDLL(lh.library_path())
+# The checking library is git-ignored and may have travelled with the tree from another build: refuse to vouch for
+# the kernel with a library that was compiled from other sources than the ones in this tree.
+from paper_2004_06352_b200 import _build  # noqa: E402
+
+lib.lh_source_hash.restype = C.c_char_p
+if lib.lh_source_hash().decode() != _build.source_hash():
+    sys.exit(f"{lh.library_path()} was built from other sources (hash {lib.lh_source_hash().decode()[:16]}..., tree "
+             f"{_build.source_hash()[:16]}...): rebuild it with __graft_entry__.build()")
 lib.lh_debug_bounds_add.argtypes = [C.c_void_p, C.c_ulonglong]
 lib.lh_debug_violations.restype = C.c_longlong
 

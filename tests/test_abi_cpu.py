@@ -15,10 +15,28 @@ import paper_2004_06352_b200 as lh
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_functions():
-    src = open(os.path.join(ROOT, "include", "lh.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(lh_[a-z0-9_]+)\s*\(", src)))
+def declared_functions(headers=("lh.h", "lh_diag.h")):
+    """every function the headers declare; the lh_debug_* calls exist in the checking build only"""
+    names = set()
+    for h in headers:
+        src = open(os.path.join(ROOT, "include", h)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        src = re.sub(r"#ifdef LH_BOUNDS_CHECK.*?#endif", "", src, flags=re.S)
+        names |= set(re.findall(r"\b(lh_[a-z0-9_]+)\s*\(", src))
+    return sorted(names)
+
+
+def test_boundary_header_holds_the_method_only():
+    """include/lh.h is the boundary of SURVEY.md sec. 8(b) and its documented extensions; probes and test hooks are
+    declared in include/lh_diag.h."""
+    method, diag = set(declared_functions(("lh.h",))), set(declared_functions(("lh_diag.h",)))
+    assert diag == {"lh_launch_count", "lh_fp64_peak_probe", "lh_math_host_eval", "lh_source_hash"}
+    assert not method & diag and not any("debug" in n or "probe" in n for n in method)
+
+
+def test_library_was_built_from_this_tree():
+    lh._build.build()
+    assert lh.lh_source_hash() == lh._build.source_hash()
 
 
 def test_library_exports_every_declared_symbol():
