@@ -13,7 +13,11 @@ One process per GPU.  The path shards with no exchange step (pixels are independ
     GPUs", Fig. 7, Table A.4): rank r evaluates rows lens_inputs.row_slab(r, N) of the ONE map with lh_grid_eval_rows
     on its own device, the whole lens list replicated; `value` = evals of the one map / the slowest rank's time.
     Assembling the map on rank 0 (one gather of the slabs) is timed separately (`assemble`), it is not part of the
-    computation.
+    computation.  For a BATCH config (--config 4) the same arm shards the other way SURVEY.md sec. 8(e) names, "for the
+    batch path, models per GPU" (one map per tested parameter set): rank r evaluates models
+    lens_inputs.model_slab(nmodel, r, N) of the ONE batch with lh_grid_gradient_batch (a pointer offset into the lens
+    array) into its slice of [nmodel][ny][nx] -- in peer mode straight into rank 0's planes; `value` = evals of the
+    whole batch / the slowest rank's time; rank 0 checks the assembled batch bitwise against its own single-device batch.
   * --scaling weak: every rank evaluates its own lens model on the full grid (independent MCMC samples).
 Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded
 sample of the same workload.
@@ -69,7 +73,8 @@ def parse():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (bench line: 3)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scaling", default="auto", choices=["auto", "strong", "weak"],
-                    help="N > 1: strong = row slabs of ONE map (default), weak = an independent lens model per rank")
+                    help="N > 1: strong (default) = ONE job over the GPUs: row slabs of the one map, or for a batch config "
+                         "(--config 4) the models of the one batch; weak = an independent job per rank")
     ap.add_argument("--assemble", default="auto", choices=["auto", "peer", "gather"],
                     help="strong scaling: how the one map reaches rank 0 -- peer: every rank's kernel stores its rows straight "
                          "into rank 0's planes (CUDA IPC + NVLink peer access, no second pass); gather: one dist.gather "
@@ -193,6 +198,9 @@ def workload_config(cfg, args, world, scaling):
     g = cfg.grid
     if world == 1:
         par = "one GPU"
+    elif scaling == "strong" and cfg.nmodel > 1:
+        par = (f"the {cfg.nmodel} models of the ONE batch over {world} GPUs (lens_inputs.model_slab, lh_grid_gradient_batch on "
+               "each rank's models), no collective in the computation; peer stores or one gather assemble the batch")
     elif scaling == "strong":
         par = (f"row slabs of the ONE map over {world} GPUs (lens_inputs.row_slab, lh_grid_eval_rows), lens list "
                "replicated, no collective in the computation; one gather assembles the map (timed apart)")
@@ -350,16 +358,24 @@ def run_ours(args):
     g = cfg.grid
     scaling = args.scaling
     if scaling == "auto":
-        scaling = "strong" if (world > 1 and cfg.nmodel == 1 and not args.stats) else "weak"
-    if scaling == "strong" and (cfg.nmodel != 1 or args.stats):
-        raise SystemExit("--scaling strong shards the rows of ONE map: use a single-model config")
+        scaling = "strong" if (world > 1 and not args.stats) else "weak"
+    if scaling == "strong" and args.stats:
+        raise SystemExit("--scaling strong: the statistics mode folds every model on one device (use --scaling weak)")
+    # split (i) rows of the ONE map, split (ii) "for the batch path, models per GPU"
+    by_model = scaling == "strong" and cfg.nmodel > 1
+    by_rows = scaling == "strong" and not by_model
+    m0, m1 = li.model_slab(cfg.nmodel, rank, world) if by_model else (0, cfg.nmodel)
+    nmine = m1 - m0
     lenses = cfg.lenses
+    lenses_mine = cfg.lenses[m0 * cfg.nlens:m1 * cfg.nlens]  # by_model: this rank's models (a pointer offset at the C ABI)
     if scaling == "weak" and world > 1 and rank > 0 and cfg.nmodel == 1:
         # another independent sample of the same model family for this rank (same shape, other seed)
         nh = {1: 2, 2: 3, 3: 4}.get(args.config, 0)
         lenses = li.cluster(1000 * args.config + rank, nh, cfg.nlens - nh, {0: 40.0, 3: 150.0}.get(args.config, 100.0))
-    j0, nrows = li.row_slab(g, rank, world) if scaling == "strong" else (0, g.ny)
-    shape = (nrows, g.nx) if scaling == "strong" else (cfg.nmodel, g.ny, g.nx)
+    j0, nrows = li.row_slab(g, rank, world) if by_rows else (0, g.ny)
+    shape = (nrows, g.nx) if by_rows else (nmine, g.ny, g.nx)
+    whole = (g.ny, g.nx) if by_rows else (cfg.nmodel, g.ny, g.nx)  # the assembled result on rank 0
+    first = j0 * g.nx if by_rows else m0 * g.npix                   # element offset of this rank's part inside it
     if args.stats:
         import dataclasses
         cfg = dataclasses.replace(cfg, outputs=("ax", "ay", "kappa", "gamma1", "gamma2"))
@@ -378,7 +394,7 @@ def run_ours(args):
         handles = [None]
         if rank == 0:
             try:
-                owner_map = {n: torch.empty((g.ny, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs}
+                owner_map = {n: torch.empty(whole, dtype=torch.float64, device="cuda") for n in cfg.outputs}
                 handles = [{n: lh.lh_ipc_export(t) for n, t in owner_map.items()}]
             except Exception as e:  # e.g. an allocator whose memory cannot be exported
                 ok, err, handles = 0, repr(e), [None]
@@ -386,12 +402,12 @@ def run_ours(args):
         if handles[0] is None:
             ok = 0
         elif rank == 0:
-            peer = {n: owner_map[n][j0:j0 + nrows] for n in cfg.outputs}
+            peer = {n: (owner_map[n][j0:j0 + nrows] if by_rows else owner_map[n][m0:m1]) for n in cfg.outputs}
         else:
             try:
                 for n in cfg.outputs:
                     peer_ptrs[n] = lh.lh_ipc_open(*handles[0][n])
-                peer = {n: peer_ptrs[n] + j0 * g.nx * 8 for n in cfg.outputs}  # address of this rank's first row
+                peer = {n: peer_ptrs[n] + first * 8 for n in cfg.outputs}  # address of this rank's first row / model
             except Exception as e:  # no peer access between the two devices: fall back to the gather
                 ok, err = 0, repr(e)
         t = torch.tensor([float(ok)], dtype=torch.float64, device=red_dev)
@@ -403,12 +419,28 @@ def run_ours(args):
                 lh.lh_ipc_close(ptr)
             peer, peer_ptrs, owner_map = None, {}, None
 
+    def run_part(target):
+        """this rank's part of the strong-scaling job into `target` (its own planes, or its place in rank 0's)"""
+        if by_rows and nrows > 0:
+            lh.lh_grid_eval_rows(lenses, g, j0, nrows, **target)
+        elif by_model and nmine > 0:
+            if tuple(cfg.outputs) == ("ax", "ay"):  # the north-star call of the batch path
+                lh.lh_grid_gradient_batch(lenses_mine, nmine, cfg.nlens, g, target["ax"], target["ay"])
+            else:
+                lh.lh_grid_eval_batch(lenses_mine, nmine, cfg.nlens, g, **target)
+
+    def run_whole(target):
+        """the whole job on this device (rank 0's bitwise reference of the assembled result)"""
+        if by_rows:
+            lh.lh_grid_eval(lenses, g, **target)
+        else:
+            lh.lh_grid_eval_batch(cfg.lenses, cfg.nmodel, cfg.nlens, g, **target)
+
     def step():
         if args.stats:
             lh.lh_grid_stats_batch(lenses, cfg.nmodel, cfg.nlens, g, out, var)
         elif scaling == "strong":
-            if nrows > 0:
-                lh.lh_grid_eval_rows(lenses, g, j0, nrows, **(peer if peer is not None else out))
+            run_part(peer if peer is not None else out)
         else:
             lh.lh_grid_eval_batch(lenses, cfg.nmodel, cfg.nlens, g, **out)
 
@@ -441,16 +473,16 @@ def run_ours(args):
     # ---- strong scaling, peer mode: the timed steps already left the whole map in rank 0's planes
     assemble = None
     if peer is not None:
-        if nrows > 0:
-            lh.lh_grid_eval_rows(lenses, g, j0, nrows, **out)  # this rank's own copy (parity sample, e2e comparison)
+        run_part(out)  # this rank's own copy (parity sample, e2e comparison)
         barrier()  # every writer synchronised: the owner may read
-        assemble = {"ms": 0.0, "bytes": int(len(cfg.outputs) * g.npix * 8), "mode": "peer",
-                    "how": "every rank's lh_grid_eval_rows stores its rows straight into rank 0's planes (CUDA IPC mapping, "
-                           "peer access over NVLink): the assembly is inside the timed steps, no gather, no second pass",
+        assemble = {"ms": 0.0, "bytes": int(len(cfg.outputs) * int(np.prod(whole)) * 8), "mode": "peer",
+                    "how": ("every rank's kernels store its " + ("rows" if by_rows else "models") + " straight into rank 0's planes "
+                            "(CUDA IPC mapping, peer access over NVLink): the assembly is inside the timed steps, no gather, "
+                            "no second pass"),
                     "bitwise_check": None}
         if rank == 0:
-            ref = {n: torch.empty((g.ny, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs}
-            lh.lh_grid_eval(lenses, g, **ref)
+            ref = {n: torch.empty(whole, dtype=torch.float64, device="cuda") for n in cfg.outputs}
+            run_whole(ref)
             torch.cuda.synchronize()
             assemble["bitwise_check"] = all(bool((owner_map[n].view(torch.int64) == ref[n].view(torch.int64)).all())
                                             for n in cfg.outputs)
@@ -460,19 +492,24 @@ def run_ours(args):
             lh.lh_ipc_close(ptr)
     # ---- strong scaling, gather mode: the time to assemble the one map on rank 0 (not part of the computation)
     if scaling == "strong" and world > 1 and peer is None:
-        rows_of = [li.row_slab(g, r, world)[1] for r in range(world)]
+        if by_rows:
+            rows_of = [li.row_slab(g, r, world)[1] for r in range(world)]
+            unit = (g.nx,)
+        else:  # units are whole models
+            rows_of = [b - a for a, b in (li.model_slab(cfg.nmodel, r, world) for r in range(world))]
+            unit = (g.ny, g.nx)
         pad = max(rows_of)
-        full = {n: torch.empty((world, pad, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs} if rank == 0 else None
-        mine = {n: torch.zeros((pad, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs}
+        full = {n: torch.empty((world, pad) + unit, dtype=torch.float64, device="cuda") for n in cfg.outputs} if rank == 0 else None
+        mine = {n: torch.zeros((pad,) + unit, dtype=torch.float64, device="cuda") for n in cfg.outputs}
         for n in cfg.outputs:
-            mine[n][:nrows].copy_(out[n])
+            mine[n][:rows_of[rank]].copy_(out[n])
 
         def gather():
             for n in cfg.outputs:
                 if backend == "nccl":
                     dist.gather(mine[n], list(full[n].unbind(0)) if rank == 0 else None, dst=0)
                 else:  # gloo stand-in: through host memory
-                    parts = [torch.empty((pad, g.nx), dtype=torch.float64) for _ in range(world)] if rank == 0 else None
+                    parts = [torch.empty((pad,) + unit, dtype=torch.float64) for _ in range(world)] if rank == 0 else None
                     dist.gather(mine[n].cpu(), parts, dst=0)
                     if rank == 0:
                         full[n].copy_(torch.stack(parts))
@@ -488,13 +525,13 @@ def run_ours(args):
         torch.cuda.synchronize()
         dev_ms = reduce_max(e0.elapsed_time(e1) / 3)
         wall_ms = reduce_max((time.perf_counter() - t0) * 1e3 / 3)
-        assemble = {"ms": dev_ms if backend == "nccl" else wall_ms, "bytes": int(len(cfg.outputs) * g.npix * 8),
+        assemble = {"ms": dev_ms if backend == "nccl" else wall_ms, "bytes": int(len(cfg.outputs) * int(np.prod(whole)) * 8),
                     "mode": "gather", "how": ("one dist.gather (NCCL) of every rank's slab of each plane into rank 0's map, CUDA events, "
                             "max over ranks" if backend == "nccl" else "gloo stand-in through host memory, wall clock"),
                     "bitwise_check": None}
         if rank == 0:  # the assembled map is the single-device map, bit for bit (checked on rank 0's own device)
-            ref = {n: torch.empty((g.ny, g.nx), dtype=torch.float64, device="cuda") for n in cfg.outputs}
-            lh.lh_grid_eval(lenses, g, **ref)
+            ref = {n: torch.empty(whole, dtype=torch.float64, device="cuda") for n in cfg.outputs}
+            run_whole(ref)
             torch.cuda.synchronize()
             ok = True
             for n in cfg.outputs:
@@ -523,9 +560,12 @@ def run_ours(args):
                         host[n].copy_(out[n], non_blocking=pinned)
                         hvar[n].copy_(var[n], non_blocking=pinned)
                     torch.cuda.synchronize()
-                elif scaling == "strong":
+                elif by_rows:
                     if nrows > 0:
                         lh.lh_grid_eval_rows_host(lenses, g, j0, nrows, **host)
+                elif by_model:
+                    if nmine > 0:
+                        lh.lh_grid_eval_host(lenses_mine, nmine, cfg.nlens, g, **host)
                 else:
                     lh.lh_grid_eval_host(lenses, cfg.nmodel, cfg.nlens, g, **host)
 
@@ -544,9 +584,9 @@ def run_ours(args):
 
         ms_pin, t_pin, bit_pin = e2e_run(True)
         ms_page, t_page, bit_page = e2e_run(False)
-        nl = cfg.nmodel * cfg.nlens
+        nl = nmine * cfg.nlens
         e2e = {"value": job_evals / (ms_pin * 1e-3), "unit": UNIT,
-               "h2d_bytes_per_step": int(nl * 192 + cfg.nmodel * 8),
+               "h2d_bytes_per_step": int(nl * 192 + nmine * 8),
                "d2h_bytes_per_step": int(len(cfg.outputs) * g.npix * 16 if args.stats else
                                          len(cfg.outputs) * int(np.prod(shape)) * 8),
                "ms_per_step": ms_pin, "steps": k_e2e, **{k: v for k, v in stats_of(t_pin).items() if k != "n"},
@@ -554,7 +594,7 @@ def run_ours(args):
                "pageable": {"value": job_evals / (ms_page * 1e-3), "ms_per_step": ms_page, "steps": k_e2e,
                             **{k: v for k, v in stats_of(t_page).items() if k != "n"},
                             "same_bits_as_device_planes": bit_page},
-               "note": ("lh_grid_eval_rows_host" if scaling == "strong" else "lh_grid_eval_host")
+               "note": ("lh_grid_eval_rows_host" if by_rows else "lh_grid_eval_host")
                        + ": host lens list in, host planes out, validation + packing + copies + sync timed (wall clock "
                          "around the call, max over ranks); the D2H copy of each of up to 8 pieces overlaps the computation "
                          "of the next; bytes are per rank"}
@@ -571,7 +611,7 @@ def run_ours(args):
     fpe = FLOPS_PER_EVAL[mode]
     step_s = float(np.mean(step_ms)) * 1e-3      # rank 0's own steps
     per_step = launches / args.steps
-    rank_evals = cfg.evals * (nrows / g.ny if scaling == "strong" else 1.0)
+    rank_evals = cfg.evals * (nrows / g.ny if by_rows else (nmine / cfg.nmodel if by_model else 1.0))
     launch_s = step_s / max(per_step, 1e-9)       # average duration of one superpose_kernel launch (CUDA events)
     launch_evals = rank_evals / max(per_step, 1e-9)  # units one launch processes
     achieved = fpe * launch_evals / launch_s / 1e12
@@ -604,9 +644,9 @@ def run_ours(args):
     if world > 1:
         line["gpu_launches_rank0"] = int(launches)
     if not args.stats:
-        sub = cfg if scaling != "strong" else None
-        if sub is not None:
-            line["parity_last_step"] = sampled_parity(torch, cfg, out, model=cfg.nmodel - 1)
+        sub = cfg if not by_rows else None
+        if sub is not None:  # rank 0 holds models [0, nmine): local and global model index agree
+            line["parity_last_step"] = sampled_parity(torch, cfg, out, model=nmine - 1)
         else:  # rank 0's slab: rows [0, nrows) of the same grid
             import dataclasses
             slab = dataclasses.replace(cfg, grid=li.Grid(g.x0, g.y0, g.dx, g.nx, nrows))

@@ -651,6 +651,40 @@ def test_bench_strong_scaling_arm_two_ranks_over_gloo(assemble):
     assert abs(d["value"] - d["config"]["evals_per_step"] / (d["ms_per_step"] * 1e-3)) < 1e-6 * d["value"]
 
 
+@pytest.mark.parametrize("assemble", ["peer", "gather"])
+def test_bench_by_model_split_of_the_batch_two_ranks_over_gloo(assemble):
+    """SURVEY sec. 8(e) split (ii), "for the batch path, models per GPU", through the product and the bench:
+    `bench.py --config 4 --gpus 2` (two ranks on this one GPU, process group on gloo) gives rank r the models
+    lens_inputs.model_slab(64, r, 2) of the ONE batch via lh_grid_gradient_batch; the assembled [64][ny][nx] planes
+    on rank 0 equal its own single-device batch bit for bit; `value` counts the batch once."""
+    import json
+    import socket
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    env = dict(os.environ, LH_BENCH_BACKEND="gloo")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "3",
+           "--warmup", "3", "--config", "4", "--no-cpu-baseline", "--assemble", assemble]
+    r = subprocess.run(cmd, env=env, cwd=root, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout[-2000:]
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "strong" and "model_slab" in d["config"]["parallelism"]
+    # 300 lenses = 2 launches per model; 32 models per rank and step
+    assert d["gpu_launches"] == 3 * 64 * 2 and d["gpu_launches_rank0"] == 3 * 32 * 2
+    assert d["assemble"]["mode"] == assemble
+    assert d["assemble"]["bitwise_check"] is True and d["assemble"]["bytes"] == 2 * 64 * 1024 * 1024 * 8
+    assert d["parity_last_step"]["ok"] and d["e2e"]["same_bits_as_device_planes"] is True
+    assert d["config"]["evals_per_step"] == 64 * 1024 * 1024 * 300
+    assert abs(d["value"] - d["config"]["evals_per_step"] / (d["ms_per_step"] * 1e-3)) < 1e-6 * d["value"]
+
+
 def test_ipc_export_open_roundtrip_in_another_process():
     """lh_ipc_export / lh_ipc_open / lh_ipc_close: a child process maps a tensor of this process (which sits INSIDE a
     larger allocation of torch's caching allocator, at a non-zero offset), lets lh_grid_eval_rows write two rows of
