@@ -63,6 +63,11 @@ FP64_LANES_PER_S = 148 * 64 * 1.965e9
 # config (profiles/r02_all_configs_ncu.md, profiles/r02_cfg3_ncu.md: a middle lens chunk where the model is chunked;
 # launches whose output fits the 126 MB L2 show almost no DRAM traffic inside the launch -- write-back caching)
 NCU_TRAFFIC_BYTES = {0: 1.04e5, 1: 1.02e5, 2: 5.44e7, 3: 6.191e8, 4: 1.688e7}
+# the NEXT-row kernels (profiles/r03_next_rows_ncu.md): delens_kernel on 4096^2 vertices x 80 sources; the statistics
+# epilogue launch (last lens chunk of a model of cfg 4 with --stats).  tests/test_profiles_cpu.py compares all of these
+# constants with the figures in the profile notes they cite.
+NCU_TRAFFIC_DELENS_BYTES = 2.725e8
+NCU_TRAFFIC_STATS_BYTES = 1.568e8
 
 
 def parse():
@@ -618,7 +623,8 @@ def run_ours(args):
     instr_rate = FP64_INSTR_PER_EVAL[mode] * launch_evals / launch_s  # FP64 thread-instructions / s
     d, m, a = FP64_OPS_PER_EVAL[mode]
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_flops / 1e12, "unit": "TFLOP/s",
-                "frac": achieved / (peak_flops / 1e12), "traffic": NCU_TRAFFIC_BYTES.get(args.config),
+                "frac": achieved / (peak_flops / 1e12),
+                "traffic": NCU_TRAFFIC_STATS_BYTES if (args.stats and args.config == 4) else NCU_TRAFFIC_BYTES.get(args.config),
                 "peak_source": "measured live: lh_fp64_peak_probe (DFMA chains, all SMs); nominal "
                                f"{NOMINAL_FP64_TFLOPS:.1f} TFLOP/s = 148 SM x 64 lanes x 2 x 1.965 GHz "
                                "(MEASURED_PEAKS.json has no FP64 entry)",
@@ -795,11 +801,13 @@ def run_delens(args):
             "config": {"workload": f"NEXT row f1: {g.nx}x{g.ny} vertices of configs[{args.config}], {ns} sources"},
             "clocks": clk.summary(), "gpu_launches": int(lh.lh_launch_count() - n0),
             "roofline": {"bound": "hbm", "achieved": 16.0 * g.npix / (ms * 1e-3) / 1e9, "peak": 6545.0, "unit": "GB/s",
-                         "frac": 16.0 * g.npix / (ms * 1e-3) / 1e9 / 6545.0, "traffic": None,
+                         "frac": 16.0 * g.npix / (ms * 1e-3) / 1e9 / 6545.0,
+                         "traffic": NCU_TRAFFIC_DELENS_BYTES if (args.config == 3 and ns == 80) else None,
                          "note": "algorithmic bytes = the two deflection planes read once (16 B per vertex); the found "
-                                 "images are a few KB.  A tile of 32 x 8 cells keeps only the sources inside the box of its "
-                                 "source-plane corners (usually none), so the per-pair work of round 1 (4 FP64 compares per "
-                                 "(cell, source), 0.20 of that ALU bound) is gone and what is left is streaming the planes; "
+                                 "images are a few KB.  A warp owns a tile of 32 x 8 cells, fetches each of its 33 x 9 vertices "
+                                 "once and keeps only the sources inside the box of their source-plane images (usually none; "
+                                 "32-bit monotone keys, redux.sync), so what is left is streaming the planes: ncu reads 268.5 MB "
+                                 "of DRAM for 268.4 MB algorithmic (profiles/r03_next_rows_ncu.md); "
                                  "peak = MEASURED_PEAKS.json hbm_gbs (copy bandwidth, of measured)"},
             "cpu_baseline": {"value": rows * (g.nx - 1) * ns / dt, "unit": "cell-source tests/s", "cores": 1,
                              "kind": "oracle", "sample": f"first {rows} cell rows, {ns} sources, {dt:.1f} s"}}

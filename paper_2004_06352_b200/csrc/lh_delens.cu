@@ -6,9 +6,9 @@
 //   "searching for the images by delensing and checking the grid for sources ... Each image found is
 //    stored ... divergent execution path"                               PAPER.md:194 (sec. 4.2)
 //
-// One thread owns one grid cell (two triangles, cut along V10-V01); a CTA owns a tile of 32 x 8 cells.
+// One lane owns one grid cell (two triangles, cut along V10-V01); a warp owns a tile of 32 x 8 cells.
 // The sources of a launch travel in the kernel parameters.  A tile first keeps the sources that fall in
-// the bounding box of ALL its cells' source-plane corners (shared memory list, typically empty); a cell
+// the bounding box of ALL its vertices' source-plane images (typically none); a cell
 // then rejects those against the box of its own four corners (that box contains the boxes of both
 // triangles, so nothing the definition accepts is lost) and only then runs, per triangle, the
 // definition of R22: closed bounding box of the three vertices AND the barycentric test.  The test arithmetic is written with the round-to-nearest intrinsics, i.e. WITHOUT FMA
@@ -69,97 +69,133 @@ __device__ __forceinline__ void test_triangle(const DelensParams &P, int s, doub
     P.images[k] = im;
 }
 
-// A CTA owns a tile of TILE_CW x TILE_CH cells (one warp per cell row, coalesced vertex loads) and walks the tiles
-// of the grid persistently.  Per tile: (1) every thread maps the four corners of its cell to the source plane and
-// takes their bounding box; (2) the boxes are reduced to the box of the TILE; (3) the threads scan the source list
-// together and keep, in shared memory, the few sources inside the tile's box; (4) every thread runs the R22 test of
-// its cell against those survivors only.  Steps (2)-(3) are a superset filter (a source outside the tile's box is
-// outside the box of each of its cells), so the images found are exactly those of the plain cell x source loop.
-constexpr int TILE_CW = 32, TILE_CH = DELENS_THREADS / 32;
+// A WARP owns a tile of TILE_CW x TILE_CH cells = (TILE_CW + 1) x (TILE_CH + 1) vertices, and there is no shared
+// memory and no block barrier.  Per tile: (1) lane l loads vertex column i0 + l for the TILE_CH + 1 vertex rows (all
+// loads issued before the first use: 18 coalesced 256-byte requests in flight per warp) and lanes 0..TILE_CH load the
+// one extra column i0 + 32 -- every vertex is fetched and mapped to the source plane ONCE per tile; (2) each lane
+// folds its vertices into a box and five shuffle steps per bound make the box of the TILE; (3) the warp scans the
+// source list 32 at a time against that box (one ballot per 32 sources).  Almost every tile ends here.  (4) For a
+// source that survives, every lane runs the R22 test of its cell in each of the tile's rows, reloading the four
+// corners (L1 hits).  Steps (2)-(3) are a superset filter -- the tile's box contains the box of each of its cells, and
+// fmin / fmax drop NaN corners, which never yield an image anyway -- so the images found are exactly those of the
+// plain cell x source loop, and the deciding arithmetic of step (4) is the definition's, untouched.
+// Round 2's kernel did the same filter per CTA with three block barriers and a one-thread reduction per tile and
+// fetched every vertex four times: 0.543 ms on 4096^2 x 80 sources, latency-bound at 0.08 of HBM.
+constexpr int TILE_CW = 32, TILE_CH = 8;
+constexpr int DELENS_WARPS = DELENS_THREADS / 32;
+#ifndef LH_DELENS_MINB
+#define LH_DELENS_MINB 4  // CTAs per SM the registers are held to (64); the first, shuffle-based version of this kernel measured 0.135 ms at 4, 0.141 at 3, 0.158 at 2
+#endif
 
-__device__ __forceinline__ double warp_min(double v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
-    return v;
+// The filter of steps (2)-(3) works on a monotone 32-bit KEY of a double instead of the double itself: the high word
+// with the sign folded in, so that x <= y implies key(x) <= key(y) (unsigned; equal keys for doubles that differ in
+// the low word only).  lo <= s <= hi therefore implies key(lo) <= key(s) <= key(hi): testing keys can only let MORE
+// sources through than testing doubles, never fewer, which is all a superset filter needs -- and keys take one
+// integer min / max per vertex and one hardware warp reduction (redux.sync) per bound, where doubles took a
+// multi-instruction fmin / fmax and ten shuffles (ncu on the first version of this kernel: 942 instructions per tile,
+// short-scoreboard stalls from the 80 shuffles on top).  NaN and infinite vertices give extreme keys = a wider box.
+__device__ __forceinline__ unsigned key32(double x) {
+    const int h = __double2hiint(x);
+    return (unsigned)h ^ ((unsigned)(h >> 31) | 0x80000000u);
 }
-__device__ __forceinline__ double warp_max(double v) {
+
+// step (4) for one cell and one source: corners 00, 10, 01, 11 in the image plane and in the source plane, the box
+// of the four corners (it contains the boxes of both triangles, so nothing the definition accepts is lost), then the
+// definition per triangle.  Rare; kept out of line so that the streaming loop stays small.
+__device__ __noinline__ void cell_test(const DelensParams &P, int s, double sx, double sy, int i, int j) {
+    const long long cell = (long long)j * (P.nx - 1) + i;
+    double T[4][2], B[4][2];
+    double lox = INFINITY, hix = -INFINITY, loy = INFINITY, hiy = -INFINITY;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-    return v;
+    for (int c = 0; c < 4; ++c) {
+        const int ii = i + (c & 1), jj = j + (c >> 1);
+        const size_t p = (size_t)jj * P.nx + ii;
+        T[c][0] = __dadd_rn(P.x0, __dmul_rn((double)ii, P.dx));
+        T[c][1] = __dadd_rn(P.y0, __dmul_rn((double)jj, P.dx));
+        B[c][0] = __dsub_rn(T[c][0], __ldg(P.ax + p));
+        B[c][1] = __dsub_rn(T[c][1], __ldg(P.ay + p));
+        lox = fmin(lox, B[c][0]); hix = fmax(hix, B[c][0]);
+        loy = fmin(loy, B[c][1]); hiy = fmax(hiy, B[c][1]);
+    }
+    if (sx < lox || sx > hix || sy < loy || sy > hiy) return;
+    test_triangle(P, s, sx, sy, T, B, 0, 1, 2, 2 * cell);
+    test_triangle(P, s, sx, sy, T, B, 3, 2, 1, 2 * cell + 1);
 }
 
 template <bool DEV_SRC>
-__global__ void __launch_bounds__(DELENS_THREADS) delens_kernel(const __grid_constant__ DelensParams P) {
-    __shared__ double s_part[TILE_CH][4];     // per-warp box: lox, hix, loy, hiy
-    __shared__ double s_box[4];               // box of the tile
-    __shared__ int s_n;                       // survivors of the current pass
-    __shared__ int s_idx[DELENS_SOURCES];     // their indices into the launch's source list
+__global__ void __launch_bounds__(DELENS_THREADS, LH_DELENS_MINB) delens_kernel(const __grid_constant__ DelensParams P) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ncx = P.nx - 1, ncy = P.ny - 1;
     const int tiles_x = (ncx + TILE_CW - 1) / TILE_CW, tiles_y = (ncy + TILE_CH - 1) / TILE_CH;
     const long long ntiles = (long long)tiles_x * tiles_y;
-    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+    for (long long tile = (long long)blockIdx.x * DELENS_WARPS + warp; tile < ntiles; tile += (long long)gridDim.x * DELENS_WARPS) {
         const int ty = (int)(tile / tiles_x), tx = (int)(tile - (long long)ty * tiles_x);
-        const int i = tx * TILE_CW + lane, j = ty * TILE_CH + warp;
-        const bool valid = i < ncx && j < ncy;
-        const long long cell = (long long)j * ncx + i;
-        double T[4][2], B[4][2];  // corners 00, 10, 01, 11 in the image plane and in the source plane
-        double lox = INFINITY, hix = -INFINITY, loy = INFINITY, hiy = -INFINITY;
-        if (valid) {
+        const int i0 = tx * TILE_CW, j0 = ty * TILE_CH;
+        // the sources of a scan step are requested one step ahead, the first before the vertices (ncu: 28 % of the samples
+        // of the version without this sat on the wait for the indexed constant-bank load; ptxas still places the first
+        // request behind the vertex loads, so the measured gain is nil -- 119 vs 121 us -- and the wait remains the top stall)
+        double sx = qnan, sy = qnan;
+        if (lane < P.nsources) {
+            sx = DEV_SRC ? __ldg(P.dsrc + 2 * lane) : P.src[lane][0];
+            sy = DEV_SRC ? __ldg(P.dsrc + 2 * lane + 1) : P.src[lane][1];
+        }
+        // (1) this lane's vertex column, rows j0 .. j0 + TILE_CH; an index outside the grid is clamped to the last vertex
+        // of the grid in that direction (a vertex of this tile: counting it twice leaves the box unchanged)
+        const int vi = i0 + lane, ci = vi < P.nx ? vi : P.nx - 1;
+        double vx[TILE_CH + 1], vy[TILE_CH + 1];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const int ii = i + (c & 1), jj = j + (c >> 1);
-                const size_t p = (size_t)jj * P.nx + ii;
-                T[c][0] = __dadd_rn(P.x0, __dmul_rn((double)ii, P.dx));
-                T[c][1] = __dadd_rn(P.y0, __dmul_rn((double)jj, P.dx));
-                B[c][0] = __dsub_rn(T[c][0], __ldg(P.ax + p));
-                B[c][1] = __dsub_rn(T[c][1], __ldg(P.ay + p));
-                lox = fmin(lox, B[c][0]); hix = fmax(hix, B[c][0]);
-                loy = fmin(loy, B[c][1]); hiy = fmax(hiy, B[c][1]);
-            }
+        for (int r = 0; r <= TILE_CH; ++r) {
+            const int cj = j0 + r < P.ny ? j0 + r : P.ny - 1;
+            const size_t p = (size_t)cj * P.nx + ci;
+            vx[r] = __ldg(P.ax + p);
+            vy[r] = __ldg(P.ay + p);
         }
-        // (2) box of the tile.  fmin / fmax drop NaN corners (a NaN deflection never yields an image: every
-        // comparison of the cell's own test below is false for it)
+        // the extra column i0 + TILE_CW: lane r takes its row r (the other lanes repeat row TILE_CH)
+        const int ei = i0 + TILE_CW < P.nx ? i0 + TILE_CW : P.nx - 1;
+        const int er = lane <= TILE_CH ? lane : TILE_CH, ej = j0 + er < P.ny ? j0 + er : P.ny - 1;
+        const double ex = __ldg(P.ax + (size_t)ej * P.nx + ei);
+        const double ey = __ldg(P.ay + (size_t)ej * P.nx + ei);
+        // (2) box of the tile's vertices in the source plane, in keys: beta = theta - alpha, theta as step (4) forms it
+        const double thx = __dadd_rn(P.x0, __dmul_rn((double)ci, P.dx));
+        unsigned lox = 0xffffffffu, hix = 0u, loy = 0xffffffffu, hiy = 0u;
+#pragma unroll
+        for (int r = 0; r <= TILE_CH; ++r) {
+            const int cj = j0 + r < P.ny ? j0 + r : P.ny - 1;
+            const unsigned kx = key32(__dsub_rn(thx, vx[r]));
+            const unsigned ky = key32(__dsub_rn(__dadd_rn(P.y0, __dmul_rn((double)cj, P.dx)), vy[r]));
+            lox = min(lox, kx); hix = max(hix, kx);
+            loy = min(loy, ky); hiy = max(hiy, ky);
+        }
         {
-            const double a = warp_min(lox), b = warp_max(hix), c = warp_min(loy), d = warp_max(hiy);
-            if (lane == 0) { s_part[warp][0] = a; s_part[warp][1] = b; s_part[warp][2] = c; s_part[warp][3] = d; }
+            const unsigned kx = key32(__dsub_rn(__dadd_rn(P.x0, __dmul_rn((double)ei, P.dx)), ex));
+            const unsigned ky = key32(__dsub_rn(__dadd_rn(P.y0, __dmul_rn((double)ej, P.dx)), ey));
+            lox = min(lox, kx); hix = max(hix, kx);
+            loy = min(loy, ky); hiy = max(hiy, ky);
         }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double a = s_part[0][0], b = s_part[0][1], c = s_part[0][2], d = s_part[0][3];
-            for (int w = 1; w < TILE_CH; ++w) {
-                a = fmin(a, s_part[w][0]); b = fmax(b, s_part[w][1]);
-                c = fmin(c, s_part[w][2]); d = fmax(d, s_part[w][3]);
+        const unsigned tlox = __reduce_min_sync(0xffffffffu, lox), thix = __reduce_max_sync(0xffffffffu, hix);
+        const unsigned tloy = __reduce_min_sync(0xffffffffu, loy), thiy = __reduce_max_sync(0xffffffffu, hiy);
+        // (3) the source list, 32 sources per step.  (A NaN source -- a chi^2 source without constraints -- has an
+        // extreme key and normally fails here; where it does not, every comparison of step (4) is false for it.)
+        for (int s0 = 0; s0 < P.nsources; s0 += 32) {
+            const int s = s0 + lane, sn = s + 32;
+            double nsx = qnan, nsy = qnan;  // the next step's sources, one step ahead
+            if (sn < P.nsources) {
+                nsx = DEV_SRC ? __ldg(P.dsrc + 2 * sn) : P.src[sn][0];
+                nsy = DEV_SRC ? __ldg(P.dsrc + 2 * sn + 1) : P.src[sn][1];
             }
-            s_box[0] = a; s_box[1] = b; s_box[2] = c; s_box[3] = d;
-        }
-        // DEV_SRC: the device list may be longer than one pass holds
-        for (int s0 = 0; s0 < P.nsources; s0 += DELENS_SOURCES) {
-            const int ns = P.nsources - s0 < DELENS_SOURCES ? P.nsources - s0 : DELENS_SOURCES;
-            if (threadIdx.x == 0) s_n = 0;
-            __syncthreads();
-            // (3) sources inside the tile's box (NaN sources -- chi^2 sources without constraints -- fail the test)
-            const double tlox = s_box[0], thix = s_box[1], tloy = s_box[2], thiy = s_box[3];
-            for (int s = threadIdx.x; s < ns; s += DELENS_THREADS) {
-                const double sx = DEV_SRC ? __ldg(P.dsrc + 2 * (s0 + s)) : P.src[s][0];
-                const double sy = DEV_SRC ? __ldg(P.dsrc + 2 * (s0 + s) + 1) : P.src[s][1];
-                if (sx >= tlox && sx <= thix && sy >= tloy && sy <= thiy) s_idx[atomicAdd(&s_n, 1)] = s;
+            const unsigned ksx = key32(sx), ksy = key32(sy);
+            unsigned m = __ballot_sync(0xffffffffu, s < P.nsources && ksx >= tlox && ksx <= thix && ksy >= tloy && ksy <= thiy);
+            // (4) rare: the cells of the tile against each survivor
+            while (m) {
+                const int b = __ffs(m) - 1;
+                m &= m - 1;
+                const double qx = __shfl_sync(0xffffffffu, sx, b), qy = __shfl_sync(0xffffffffu, sy, b);
+#pragma unroll 1
+                for (int r = 0; r < TILE_CH; ++r)
+                    if (vi < ncx && j0 + r < ncy) cell_test(P, s0 + b, qx, qy, vi, j0 + r);
             }
-            __syncthreads();
-            // (4) the cell's own test on the survivors
-            const int n = s_n;
-            if (valid) {
-                for (int q = 0; q < n; ++q) {
-                    const int s = s_idx[q];
-                    const double sx = DEV_SRC ? __ldg(P.dsrc + 2 * (s0 + s)) : P.src[s][0];
-                    const double sy = DEV_SRC ? __ldg(P.dsrc + 2 * (s0 + s) + 1) : P.src[s][1];
-                    // outside the box of the four corners = outside the box of either triangle (R22): reject
-                    if (sx < lox || sx > hix || sy < loy || sy > hiy) continue;
-                    test_triangle(P, s0 + s, sx, sy, T, B, 0, 1, 2, 2 * cell);
-                    test_triangle(P, s0 + s, sx, sy, T, B, 3, 2, 1, 2 * cell + 1);
-                }
-            }
-            __syncthreads();  // s_n / s_idx / s_box are rewritten by the next pass or tile
+            sx = nsx; sy = nsy;
         }
     }
 }
@@ -184,6 +220,14 @@ cudaError_t launch_source_plane(const double *ax, const double *ay, double x0, d
     return cudaGetLastError();
 }
 
+// One warp per tile, DELENS_WARPS tiles per CTA; beyond 64 CTAs per SM the warps walk the tiles grid-stride.
+static long long delens_blocks(int nx, int ny, int sms) {
+    const long long tiles = (long long)((nx - 1 + TILE_CW - 1) / TILE_CW) * ((ny - 1 + TILE_CH - 1) / TILE_CH);
+    long long blocks = (tiles + DELENS_WARPS - 1) / DELENS_WARPS;
+    const long long cap = (long long)(sms > 0 ? sms : 148) * 64;
+    return blocks > cap ? cap : (blocks < 1 ? 1 : blocks);
+}
+
 // sources: HOST [ns][2].  One launch per DELENS_SOURCES sources; `count` must be zero on entry.
 cudaError_t launch_delens(const double *ax, const double *ay, double x0, double y0, double dx, int nx, int ny,
                           const double *sources, int ns, lh_image *images, long long max_images,
@@ -193,8 +237,7 @@ cudaError_t launch_delens(const double *ax, const double *ay, double x0, double 
     P.x0 = x0; P.y0 = y0; P.dx = dx; P.nx = nx; P.ny = ny;
     const long long ncells = (long long)(nx - 1) * (ny - 1);
     if (ncells <= 0) return cudaSuccess;
-    long long blocks = (long long)((nx - 1 + TILE_CW - 1) / TILE_CW) * ((ny - 1 + TILE_CH - 1) / TILE_CH);
-    if (blocks > (long long)sms * 8) blocks = (long long)sms * 8;  // persistent: 8 CTAs of 256 threads per SM
+    long long blocks = delens_blocks(nx, ny, sms);
     for (int s0 = 0; s0 < ns; s0 += DELENS_SOURCES) {
         const int n = ns - s0 < DELENS_SOURCES ? ns - s0 : DELENS_SOURCES;
         P.source0 = s0; P.nsources = n;
@@ -218,8 +261,7 @@ cudaError_t launch_delens_dev(const double *ax, const double *ay, double x0, dou
     P.source0 = 0; P.nsources = ns; P.dsrc = dsources;
     const long long ncells = (long long)(nx - 1) * (ny - 1);
     if (ncells <= 0 || ns <= 0) return cudaSuccess;
-    long long blocks = (long long)((nx - 1 + TILE_CW - 1) / TILE_CW) * ((ny - 1 + TILE_CH - 1) / TILE_CH);
-    if (blocks > (long long)sms * 8) blocks = (long long)sms * 8;
+    long long blocks = delens_blocks(nx, ny, sms);
     delens_kernel<true><<<(unsigned)blocks, DELENS_THREADS, 0, st>>>(P);
     ++*launches;
     return cudaGetLastError();
