@@ -308,12 +308,38 @@ def config_block(torch, lh, stream, flush, which=(0, 1, 2, 4), steps=5, oracle_t
         mode = variant_of(c.outputs)
         st = stats_of(ms)
         sec = st["ms_median"] * 1e-3
+        # what a sampler that needs each result before its next proposal sees: host lens list in,
+        # device planes out, a synchronize after every call -- wall clock, no L2 flush (the sampler would not flush
+        # either).  Beside it the host-only share: validation + packing of all the call's lenses (lh_pack_model).
+        torch.cuda.synchronize()
+        k_sync = max(steps, 20 if c.evals < 2e9 else steps)
+        walls = []
+        for _ in range(k_sync):
+            t0 = time.perf_counter()
+            step()
+            torch.cuda.synchronize()
+            walls.append((time.perf_counter() - t0) * 1e3)
+        L = c.lenses.reshape(c.nmodel, c.nlens)
+        packs = []
+        for _ in range(5):
+            t0 = time.perf_counter()
+            for m in range(c.nmodel):
+                lh.lh_pack_model(L[m])
+            packs.append((time.perf_counter() - t0) * 1e3)
+        per_call = {"ms_median": float(np.median(walls)), "ms_best": float(np.min(walls)), "calls": k_sync,
+                    "overhead_ms": float(np.median(walls)) - st["ms_median"],
+                    "overhead_frac_of_kernel_time": float(np.median(walls)) / st["ms_median"] - 1.0,
+                    "host_pack_ms": float(np.median(packs)),
+                    "note": "one call + torch.cuda.synchronize(), wall clock (validation, packing, ctypes, launches, "
+                            "kernels, sync); overhead = that minus the device-timed median; host_pack_ms = lh_pack_model "
+                            f"over the call's {c.nmodel * c.nlens} lenses from Python, one call per model (includes "
+                            "ctypes and the table allocation: an upper bound of the packing inside the call)"}
         block[f"cfg{idx}"] = {
             "workload": f"{c.name}: {g.nx}x{g.ny} px x {c.nlens} lenses" + (f" x {c.nmodel} models" if c.nmodel > 1 else ""),
             "outputs": list(c.outputs), "kernel": f"superpose_kernel<{mode}>", "steps": steps, **st,
             "evals_per_s": c.evals / sec, "launches_per_step": launches / steps,
             "fp64_issue_frac": fp64_instr_of(c, mode) * g.npix * c.nmodel / sec / FP64_LANES_PER_S,
-            "traffic": NCU_TRAFFIC_BYTES.get(idx),
+            "traffic": NCU_TRAFFIC_BYTES.get(idx), "per_call_synchronised": per_call,
             "parity_last_step": sampled_parity(torch, c, out, model=c.nmodel - 1, n=300)}
         del out
         if oracle_too:
